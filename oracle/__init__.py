@@ -1,0 +1,10 @@
+"""CPU oracle -- TEST INFRASTRUCTURE, NOT THE PRODUCT (see oracle_eigh.c).
+
+Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference
+legs may import this package.  paper_2310_03341_b200 never does.
+"""
+from .oracle import (build, eigh, eigh_ld, tridiagonalise, tridiag_ql, tridiag_ql_ld,
+                     num_threads)
+
+__all__ = ["build", "eigh", "eigh_ld", "tridiagonalise", "tridiag_ql", "tridiag_ql_ld",
+           "num_threads"]
