@@ -1,0 +1,149 @@
+/* eigh.h -- C ABI of b200-eigh: dense complex-FP64 Hermitian eigensolver for one B200 (sm_100a).
+ *
+ * The operation is the Hermitian eigenproblem of the paper's Eq. 7:
+ * find real E_0 <= ... <= E_{N-1} and an orthonormal set phi_n with  H phi_n = E_n phi_n,
+ * for the dense BdG/HFB Hamiltonian H ("dense diagonalization").  The method
+ * is the 2-stage solver outlined in PAPER.md:148-154: dense -> band -> tridiagonal,
+ * tridiagonal eigensolve, and a two-stage back-transformation of the eigenvectors.
+ * Everything below the five named steps is this library's own design.
+ *
+ * Conventions
+ *   - All pointers named *_dev are DEVICE pointers; everything else is host memory.
+ *   - Matrices are column-major; complex elements are interleaved (re, im) FP64 pairs
+ *     ("c128", 16 bytes); leading dimensions are in ELEMENTS.
+ *   - `stream` is a cudaStream_t passed as void* (0 = default stream).  Calls enqueue work
+ *     on that stream only and may synchronise it (documented per call).
+ *   - Return value: 0 success; -k = k-th argument invalid (nothing launched);
+ *     +k = numerical failure count reported after completion (e.g. secular iterations that
+ *     did not converge); EIGH_ERR_CUDA (= 1000 + cudaError_t) on a CUDA runtime error.
+ *     eigh_last_error(h) gives a text description.
+ *   - Ownership: the caller owns A, W, Z and the workspace (e.g. torch tensors); the handle
+ *     owns only host-side plan data and a few CUDA events.  One handle per host thread.
+ *   - There is NO CPU fallback anywhere in this library.
+ */
+#ifndef EIGH_B200_H
+#define EIGH_B200_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define EIGH_ERR_CUDA 1000
+
+typedef struct eigh_handle_s* eigh_handle_t;
+
+/* Plan a solve of order N returning the LOWEST nev eigenpairs (1 <= nev <= N; "all or the
+ * lowest nev", PAPER.md:119-127 keeps only part of the spectrum).  No device allocation.
+ * Defaults: band width b = 64, D&C leaf 32, WY group g = 64. */
+int eigh_create(eigh_handle_t* h, int64_t N, int64_t nev);
+
+/* Tuning knobs; must be called before eigh_workspace_size.  Keys: "band_width" (64 or 128),
+ * "wy_group" (16..64, <= band_width), "dc_leaf" (8..32), "p4b_merge" (1..4 panels per WY block).
+ * Returns -2 for an unknown key, -3 for a bad value. */
+int eigh_set_option(eigh_handle_t h, const char* key, int64_t value);
+
+/* Bytes of device workspace the caller must provide for this plan. */
+size_t eigh_workspace_size(eigh_handle_t h);
+
+/* Hand the workspace (device memory, 256-byte aligned, >= eigh_workspace_size bytes) to the
+ * handle.  The caller keeps ownership and must keep it alive across eigh_solve calls. */
+int eigh_set_workspace(eigh_handle_t h, void* ws_dev, size_t bytes);
+
+/* Full solve (band reduction, band -> tridiagonal, tridiagonal eigensolve,
+ * two back-transformations).
+ *   A_dev : N x N c128, lda >= N.  Only the LOWER triangle is read; imaginary parts of the
+ *           diagonal are ignored.  OVERWRITTEN (holds the stage-1 reflectors afterwards).
+ *   W_dev : N doubles, all eigenvalues ascending.
+ *   Z_dev : N x nev c128, ldz = N; column j = unit-2-norm eigenvector of W[j] (phase free).
+ * Enqueues on `stream`; synchronises `stream` before returning (so that the failure count
+ * can be returned). */
+int eigh_solve(eigh_handle_t h, void* A_dev, int64_t lda, double* W_dev, void* Z_dev,
+               void* stream);
+
+/* Per-phase device times of the last eigh_solve, in ms, from CUDA events on the solve's
+ * stream: ms[0] = full->band, [1] = band->tridiagonal, [2] = tridiagonal D&C,
+ * [3] = band back-transform, [4] = full back-transform. */
+int eigh_phase_times(eigh_handle_t h, double ms[5]);
+
+/* Kernel launches issued by the last eigh_solve (all are this library's own kernels). */
+int64_t eigh_launch_count(eigh_handle_t h);
+
+const char* eigh_last_error(eigh_handle_t h);
+int eigh_destroy(eigh_handle_t h);
+
+/* ---------------------------------------------------------------------------------------
+ * Phase-level entry points (same conventions).  They use the handle's workspace exactly as
+ * eigh_solve does, so a sequence reduce_to_band -> band_to_tridiag -> tridiag_dc ->
+ * backtransform_band -> backtransform_full on one handle reproduces eigh_solve.
+ * ------------------------------------------------------------------------------------- */
+
+/* S1 ("transforming the dense matrix in a banded matrix"): unitary Q1 with
+ * Q1^H A Q1 = B, B Hermitian of half-bandwidth b.  A_dev is overwritten: column block p
+ * holds V_p (unit lower trapezoidal, explicit ones and zeros) in rows >= (p+1) b.
+ * band_dev: (ldab x N) c128, ldab >= 2b+1... lower band storage band[i-j + j*ldab] = B[i,j]
+ * for j <= i <= min(N-1, j+b); rows b+1..ldab-1 are zeroed (bulge-chasing fill-in room). */
+int eigh_reduce_to_band(eigh_handle_t h, void* A_dev, int64_t lda, void* band_dev,
+                        int64_t ldab, void* stream);
+
+/* S2 ("transforming the banded matrix into a tridiagonal form"): unitary Q2
+ * with Q2^H B Q2 = T real symmetric tridiagonal.  band_dev (as written by S1) is destroyed.
+ * d_dev[N], e_dev[N-1] (e >= 0).  The reflectors, their taus and the phase vector stay in
+ * the workspace for S4a. */
+int eigh_band_to_tridiag(eigh_handle_t h, void* band_dev, int64_t ldab, double* d_dev,
+                         double* e_dev, void* stream);
+
+/* S3 ("diagonalizing this tridiagonal form"), divide and conquer on the GPU.
+ * d_dev[N], e_dev[N-1] are read (not modified).  W_dev[N] ascending.  Q_dev: N x nev real
+ * FP64, ldq >= N, column j = eigenvector of W[j]; may alias no other argument.
+ * Synchronises `stream`.  Returns the number of secular roots that failed to converge. */
+int eigh_tridiag_dc(eigh_handle_t h, const double* d_dev, const double* e_dev, double* W_dev,
+                    double* Q_dev, int64_t ldq, void* stream);
+
+/* S4a (first of the "two stages"): Z <- Q2 * (phase o Q_T).
+ * Q_dev: N x nev real (from S3); Z_dev: N x nev c128, ldz >= N. */
+int eigh_backtransform_band(eigh_handle_t h, const double* Q_dev, int64_t ldq, void* Z_dev,
+                            int64_t ldz, void* stream);
+
+/* S4b (second stage): Z <- Q1 * Z with the reflectors S1 left in A_dev. */
+int eigh_backtransform_full(eigh_handle_t h, const void* A_dev, int64_t lda, void* Z_dev,
+                            int64_t ldz, void* stream);
+
+/* ---------------------------------------------------------------------------------------
+ * Kernel-level entry points (unit tests and microbenchmarks of the building blocks).
+ * ------------------------------------------------------------------------------------- */
+
+/* Complex-FP64 GEMM on the FP64 tensor-core path (mma.sync m8n8k4 f64 -> DMMA):
+ *   C <- alpha * opA(A) * opB(B) [+ alpha * opA(A2) * opB(B2)] + beta * C
+ * opX = 'N' (as stored) or 'C' (conjugate transpose).  C is M x N, inner dimension K (K2 for
+ * the optional second pair; pass A2_dev = NULL to disable).  lower_only bit 0 skips output
+ * tiles that lie strictly above the diagonal (HER2K-lower); bit 1 forces the 64x64 tile
+ * configuration (default: 128x64, or 64x64 when M <= 64).  splitk >= 1 partitions K over
+ * thread blocks with a deterministic two-pass reduction (partials in the handle workspace). */
+int eigh_k_zgemm(eigh_handle_t h, char opA, char opB, int64_t M, int64_t N, int64_t K,
+                 double alpha, const void* A_dev, int64_t lda, const void* B_dev, int64_t ldb,
+                 int64_t K2, const void* A2_dev, int64_t lda2, const void* B2_dev, int64_t ldb2,
+                 double beta, void* C_dev, int64_t ldc, int lower_only, int splitk, void* stream);
+
+/* HEMM-lower on the DMMA path: C (M x N) <- Herm(A) * B, A is M x M Hermitian of which only
+ * the lower triangle AND the 64-aligned diagonal blocks are read as stored. */
+int eigh_k_zhemm_lower(eigh_handle_t h, int64_t M, int64_t N, const void* A_dev, int64_t lda,
+                       const void* B_dev, int64_t ldb, void* C_dev, int64_t ldc, int splitk,
+                       void* stream);
+
+/* Real FP64 GEMM on the DMMA path: C (M x N) <- A[:, idx] * B, K inner; a_col_idx_dev may be
+ * NULL (identity) or K int32 column indices into A. */
+int eigh_k_dgemm(eigh_handle_t h, int64_t M, int64_t N, int64_t K, const double* A_dev,
+                 int64_t lda, const int32_t* a_col_idx_dev, const double* B_dev, int64_t ldb,
+                 double* C_dev, int64_t ldc, void* stream);
+
+/* Register-resident DMMA / DFMA peak microbenchmarks: run `iters` dependent-chain-free
+ * instructions per thread on every SM; returns achieved real TFLOP/s in *tflops (host). */
+int eigh_k_fp64_peak(int use_dmma, int64_t iters, double* tflops, double* ms, void* stream);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* EIGH_B200_H */

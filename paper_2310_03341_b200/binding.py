@@ -1,0 +1,200 @@
+"""Thin ctypes binding of the C ABI in include/eigh.h (argument marshalling only).
+
+Every step of the path runs in the CUDA library; PyTorch is used for device memory and
+streams.  There is no fallback: if libeigh_b200.so is missing or fails to load, every
+entry point raises.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+from typing import Optional
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libeigh_b200.so")
+_lib = None
+
+_i64, _int, _dbl, _vp, _sz = ctypes.c_int64, ctypes.c_int, ctypes.c_double, ctypes.c_void_p, ctypes.c_size_t
+_dp = ctypes.POINTER(ctypes.c_double)
+
+# name -> (restype, argtypes); must list every function declared in include/eigh.h
+SIGNATURES = {
+    "eigh_create": (_int, [ctypes.POINTER(_vp), _i64, _i64]),
+    "eigh_set_option": (_int, [_vp, ctypes.c_char_p, _i64]),
+    "eigh_workspace_size": (_sz, [_vp]),
+    "eigh_set_workspace": (_int, [_vp, _vp, _sz]),
+    "eigh_solve": (_int, [_vp, _vp, _i64, _vp, _vp, _vp]),
+    "eigh_phase_times": (_int, [_vp, _dp]),
+    "eigh_launch_count": (_i64, [_vp]),
+    "eigh_last_error": (ctypes.c_char_p, [_vp]),
+    "eigh_destroy": (_int, [_vp]),
+    "eigh_reduce_to_band": (_int, [_vp, _vp, _i64, _vp, _i64, _vp]),
+    "eigh_band_to_tridiag": (_int, [_vp, _vp, _i64, _vp, _vp, _vp]),
+    "eigh_tridiag_dc": (_int, [_vp, _vp, _vp, _vp, _vp, _i64, _vp]),
+    "eigh_backtransform_band": (_int, [_vp, _vp, _i64, _vp, _i64, _vp]),
+    "eigh_backtransform_full": (_int, [_vp, _vp, _i64, _vp, _i64, _vp]),
+    "eigh_k_zgemm": (_int, [_vp, ctypes.c_char, ctypes.c_char, _i64, _i64, _i64, _dbl, _vp, _i64, _vp, _i64,
+                            _i64, _vp, _i64, _vp, _i64, _dbl, _vp, _i64, _int, _int, _vp]),
+    "eigh_k_zhemm_lower": (_int, [_vp, _i64, _i64, _vp, _i64, _vp, _i64, _vp, _i64, _int, _vp]),
+    "eigh_k_dgemm": (_int, [_vp, _i64, _i64, _i64, _vp, _i64, _vp, _vp, _i64, _vp, _i64, _vp]),
+    "eigh_k_fp64_peak": (_int, [_int, _i64, _dp, _dp, _vp]),
+}
+
+
+def load():
+    """Load the CUDA library; raises (loudly) if it is missing -- there is no fallback."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(LIB_PATH):
+            raise RuntimeError(
+                f"{LIB_PATH} not found: build it with `python -c 'import __graft_entry__ as g; g.build()'` "
+                "(b200-eigh has no CPU fallback)")
+        lib = ctypes.CDLL(LIB_PATH)
+        for name, (res, args) in SIGNATURES.items():
+            f = getattr(lib, name)
+            f.restype = res
+            f.argtypes = args
+        _lib = lib
+    return _lib
+
+
+class EighError(RuntimeError):
+    pass
+
+
+def _ptr(t):
+    return ctypes.c_void_p(t.data_ptr()) if t is not None else None
+
+
+def _stream():
+    import torch
+    return ctypes.c_void_p(torch.cuda.current_stream().cuda_stream)
+
+
+class Eigh:
+    """Handle + workspace for one problem size.  A is N x N complex128 with COLUMN-MAJOR
+    storage: pass a torch tensor `At` of shape (N, N) holding A^T row-major (i.e. `At[j, i] =
+    A[i, j]`), which is the same memory as A column-major."""
+
+    def __init__(self, N: int, nev: Optional[int] = None, device="cuda", **options):
+        import torch
+        self.lib = load()
+        self.N = int(N)
+        self.nev = int(nev if nev is not None else N)
+        self.device = torch.device(device)
+        h = ctypes.c_void_p()
+        rc = self.lib.eigh_create(ctypes.byref(h), self.N, self.nev)
+        if rc != 0:
+            raise EighError(f"eigh_create({N}, {nev}) -> {rc}")
+        self.h = h
+        for k, v in options.items():
+            rc = self.lib.eigh_set_option(self.h, k.encode(), int(v))
+            if rc != 0:
+                raise EighError(f"eigh_set_option({k}, {v}) -> {rc}: {self.last_error()}")
+        self.ws_bytes = int(self.lib.eigh_workspace_size(self.h))
+        self.ws = torch.empty(self.ws_bytes + 256, dtype=torch.uint8, device=self.device)
+        base = self.ws.data_ptr()
+        self._ws_ptr = (base + 255) // 256 * 256
+        rc = self.lib.eigh_set_workspace(self.h, ctypes.c_void_p(self._ws_ptr), self.ws_bytes)
+        self._check(rc, "eigh_set_workspace")
+
+    # ------------------------------------------------------------------ plumbing
+    def last_error(self) -> str:
+        return self.lib.eigh_last_error(self.h).decode()
+
+    def _check(self, rc, what, allow_positive=False):
+        if rc < 0 or rc >= 1000 or (rc > 0 and not allow_positive):
+            raise EighError(f"{what} -> {rc}: {self.last_error()}")
+        return rc
+
+    def close(self):
+        if getattr(self, "h", None):
+            self.lib.eigh_destroy(self.h)
+            self.h = None
+            self.ws = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    # ------------------------------------------------------------------ full solve
+    def solve(self, At, W=None, Zt=None):
+        """eigh_solve.  At: (N, N) complex128 CUDA tensor = A^T row-major (A column-major); it
+        is OVERWRITTEN.  Returns (W [N] float64, Zt [(nev, N)] complex128 with Zt[j] = eigenvector
+        j, i.e. Z column-major).  Positive return codes (non-converged secular roots) raise."""
+        import torch
+        assert At.is_cuda and At.dtype == torch.complex128 and At.is_contiguous() and At.shape == (self.N, self.N)
+        if W is None:
+            W = torch.empty(self.N, dtype=torch.float64, device=At.device)
+        if Zt is None:
+            Zt = torch.empty((self.nev, self.N), dtype=torch.complex128, device=At.device)
+        rc = self.lib.eigh_solve(self.h, _ptr(At), self.N, _ptr(W), _ptr(Zt), _stream())
+        self._check(rc, "eigh_solve")
+        return W, Zt
+
+    def phase_times_ms(self):
+        ms = (ctypes.c_double * 5)()
+        self.lib.eigh_phase_times(self.h, ms)
+        return list(ms)
+
+    def launch_count(self) -> int:
+        return int(self.lib.eigh_launch_count(self.h))
+
+    # ------------------------------------------------------------------ phases
+    @property
+    def ldab(self) -> int:
+        return 2 * self.band_width + 2
+
+    @property
+    def band_width(self) -> int:
+        return getattr(self, "_b", 64)
+
+    def reduce_to_band(self, At, band):
+        rc = self.lib.eigh_reduce_to_band(self.h, _ptr(At), self.N, _ptr(band), band.shape[1], _stream())
+        self._check(rc, "eigh_reduce_to_band")
+
+    def band_to_tridiag(self, band, d, e):
+        rc = self.lib.eigh_band_to_tridiag(self.h, _ptr(band), band.shape[1], _ptr(d), _ptr(e), _stream())
+        self._check(rc, "eigh_band_to_tridiag")
+
+    def tridiag_dc(self, d, e, W, Qt):
+        """Qt: (nev, ldq) float64 row-major = Q column-major with ldq = Qt.shape[1]."""
+        rc = self.lib.eigh_tridiag_dc(self.h, _ptr(d), _ptr(e), _ptr(W), _ptr(Qt), Qt.shape[1], _stream())
+        return self._check(rc, "eigh_tridiag_dc", allow_positive=True)
+
+    def backtransform_band(self, Qt, Zt):
+        rc = self.lib.eigh_backtransform_band(self.h, _ptr(Qt), Qt.shape[1], _ptr(Zt), Zt.shape[1], _stream())
+        self._check(rc, "eigh_backtransform_band")
+
+    def backtransform_full(self, At, Zt):
+        rc = self.lib.eigh_backtransform_full(self.h, _ptr(At), self.N, _ptr(Zt), Zt.shape[1], _stream())
+        self._check(rc, "eigh_backtransform_full")
+
+    # ------------------------------------------------------------------ kernels
+    def zgemm(self, opA, opB, M, N, K, alpha, A, lda, B, ldb, beta, C, ldc, K2=0, A2=None, lda2=0,
+              B2=None, ldb2=0, lower_only=0, splitk=1):
+        rc = self.lib.eigh_k_zgemm(self.h, opA.encode(), opB.encode(), M, N, K, alpha, _ptr(A), lda, _ptr(B),
+                                   ldb, K2, _ptr(A2), lda2, _ptr(B2), ldb2, beta, _ptr(C), ldc, lower_only,
+                                   splitk, _stream())
+        self._check(rc, "eigh_k_zgemm")
+
+    def zhemm_lower(self, M, N, A, lda, B, ldb, C, ldc, splitk=1):
+        rc = self.lib.eigh_k_zhemm_lower(self.h, M, N, _ptr(A), lda, _ptr(B), ldb, _ptr(C), ldc, splitk, _stream())
+        self._check(rc, "eigh_k_zhemm_lower")
+
+    def dgemm(self, M, N, K, A, lda, B, ldb, C, ldc, col_idx=None):
+        rc = self.lib.eigh_k_dgemm(self.h, M, N, K, _ptr(A), lda, _ptr(col_idx), _ptr(B), ldb, _ptr(C), ldc,
+                                   _stream())
+        self._check(rc, "eigh_k_dgemm")
+
+
+def fp64_peak(use_dmma: bool, iters: int = 20000):
+    """(TFLOP/s, ms) of the register-resident DMMA (or DFMA) loop on the current device."""
+    lib = load()
+    tf, ms = ctypes.c_double(), ctypes.c_double()
+    rc = lib.eigh_k_fp64_peak(1 if use_dmma else 0, iters, ctypes.byref(tf), ctypes.byref(ms), _stream())
+    if rc != 0:
+        raise EighError(f"eigh_k_fp64_peak -> {rc}")
+    return tf.value, ms.value

@@ -1,0 +1,400 @@
+// api.cu -- C ABI (include/eigh.h): handle, workspace plan, eigh_solve, kernel-level entry points.
+#include <stdarg.h>
+#include <stdlib.h>
+
+#include <new>
+
+#include "dgemm.cuh"
+#include "eigh_internal.h"
+#include "zgemm.cuh"
+
+namespace eigh {
+
+int set_err(eigh_handle_s* h, int code, const char* fmt, ...) {
+    if (h) {
+        va_list ap;
+        va_start(ap, fmt);
+        vsnprintf(h->err, sizeof(h->err), fmt, ap);
+        va_end(ap);
+    }
+    return code;
+}
+
+static size_t bump(size_t& off, size_t bytes) {
+    const size_t at = off;
+    off += (bytes + 255) / 256 * 256;
+    return at;
+}
+
+size_t dc_arena_bytes(int64_t N);   // tridiag_dc.cu
+size_t bt_scratch_bytes(const eigh_handle_s* h);   // backtransform.cu
+
+void plan_workspace(eigh_handle_s* h) {
+    WsPlan& p = h->plan;
+    const int64_t N = h->N, b = h->b;
+    size_t off = 0;
+    h->ldab = 2 * b + 2;
+    p.gemm_partial_bytes = (size_t)192 << 20;
+    p.gemm_partial = bump(off, p.gemm_partial_bytes);
+    p.band = bump(off, (size_t)h->ldab * N * sizeof(c128));
+    p.tau1 = bump(off, (size_t)N * sizeof(c128));
+    const int64_t npanels = ceil_div(N, b);
+    p.T1 = bump(off, (size_t)npanels * b * b * sizeof(c128));
+    p.Vp = bump(off, (size_t)N * b * sizeof(c128));
+    p.VT = bump(off, (size_t)N * b * sizeof(c128));
+    p.X = bump(off, (size_t)N * b * sizeof(c128));
+    p.small = bump(off, (size_t)4 * b * b * sizeof(c128));
+    p.panel_sync = bump(off, (size_t)(256 + 2 * 160 * (2 * b + 8) * sizeof(c128)));
+    p.V2 = bump(off, (size_t)(N * (N - 1) / 2 + 2 * b) * sizeof(c128));
+    p.bc_progress = bump(off, (size_t)(N + 8) * sizeof(int));
+    p.d = bump(off, (size_t)N * sizeof(double));
+    p.e = bump(off, (size_t)N * sizeof(double));
+    p.sgn = bump(off, (size_t)N * sizeof(double));
+    p.dc_bytes = dc_arena_bytes(N);
+    p.dc = bump(off, p.dc_bytes);
+    p.Qt = p.dc;   // the D&C driver leaves its result at the start of the arena
+    // back-transform scratch aliases the tail of the D&C arena (U and the dead Q buffer)
+    p.bt_bytes = bt_scratch_bytes(h);
+    p.bt = bump(off, p.bt_bytes);
+    p.total = off;
+    h->planned = true;
+}
+
+}  // namespace eigh
+
+using namespace eigh;
+
+extern "C" {
+
+int eigh_create(eigh_handle_t* out, int64_t N, int64_t nev) {
+    if (!out) return -1;
+    *out = nullptr;
+    if (N < 1 || N > (int64_t)1 << 20) return -2;
+    if (nev < 1 || nev > N) return -3;
+    eigh_handle_s* h = new (std::nothrow) eigh_handle_s();
+    if (!h) return -1;
+    memset(h, 0, sizeof(*h));
+    h->N = N;
+    h->nev = nev;
+    h->b = 64;
+    h->g = 64;
+    h->leaf = 32;
+    h->p4b_merge = 1;
+    h->num_sms = 0;
+    snprintf(h->err, sizeof(h->err), "ok");
+    *out = h;
+    return 0;
+}
+
+int eigh_set_option(eigh_handle_t h, const char* key, int64_t value) {
+    if (!h) return -1;
+    if (!key) return -2;
+    if (!strcmp(key, "band_width")) {
+        if (value != 64 && value != 128) return set_err(h, -3, "band_width must be 64 or 128");
+        h->b = (int)value;
+        if (h->g > h->b) h->g = h->b;
+    } else if (!strcmp(key, "wy_group")) {
+        if (value < 8 || value > 64 || value > h->b || value % 8) return set_err(h, -3, "wy_group must be a multiple of 8 in [8, min(64, band_width)]");
+        h->g = (int)value;
+    } else if (!strcmp(key, "dc_leaf")) {
+        if (value < 4 || value > 32) return set_err(h, -3, "dc_leaf must be in [4, 32]");
+        h->leaf = (int)value;
+    } else if (!strcmp(key, "p4b_merge")) {
+        if (value < 1 || value > 4) return set_err(h, -3, "p4b_merge must be in [1, 4]");
+        h->p4b_merge = (int)value;
+    } else {
+        return set_err(h, -2, "unknown option '%s'", key);
+    }
+    h->planned = false;
+    return 0;
+}
+
+size_t eigh_workspace_size(eigh_handle_t h) {
+    if (!h) return 0;
+    plan_workspace(h);
+    return h->plan.total;
+}
+
+int eigh_set_workspace(eigh_handle_t h, void* ws_dev, size_t bytes) {
+    if (!h) return -1;
+    if (!h->planned) plan_workspace(h);
+    if (!ws_dev || ((uintptr_t)ws_dev & 255)) return set_err(h, -2, "workspace must be a 256-byte aligned device pointer");
+    if (bytes < h->plan.total) return set_err(h, -3, "workspace too small: %zu < %zu", bytes, h->plan.total);
+    h->ws = ws_dev;
+    h->ws_bytes = bytes;
+    return 0;
+}
+
+static int ensure_ready(eigh_handle_t h) {
+    if (!h) return -1;
+    if (!h->ws) return set_err(h, -1, "no workspace set (call eigh_set_workspace)");
+    if (!h->planned) return set_err(h, -1, "options changed after eigh_set_workspace; call eigh_workspace_size / eigh_set_workspace again");
+    if (!h->events_ok) {
+        for (int i = 0; i < 6; ++i) {
+            cudaError_t e = cudaEventCreate(&h->ev[i]);
+            if (e != cudaSuccess) return set_err(h, 1000 + (int)e, "cudaEventCreate: %s", cudaGetErrorString(e));
+        }
+        h->events_ok = true;
+    }
+    if (!h->num_sms) {
+        int dev = 0;
+        cudaGetDevice(&dev);
+        cudaDeviceGetAttribute(&h->num_sms, cudaDevAttrMultiProcessorCount, dev);
+        if (h->num_sms <= 0) return set_err(h, EIGH_ERR_CUDA, "no CUDA device");
+    }
+    return 0;
+}
+
+static int cuda_fail(eigh_handle_t h, int rc, const char* where) {
+    if (rc >= 1000) return set_err(h, rc, "%s: CUDA error %d (%s)", where, rc - 1000, cudaGetErrorString((cudaError_t)(rc - 1000)));
+    return rc;
+}
+
+int eigh_reduce_to_band(eigh_handle_t h, void* A_dev, int64_t lda, void* band_dev, int64_t ldab, void* stream) {
+    int rc = ensure_ready(h);
+    if (rc) return rc;
+    if (!A_dev) return -2;
+    if (lda < h->N) return -3;
+    if (!band_dev) return -4;
+    if (ldab < h->ldab) return set_err(h, -5, "ldab must be >= %lld", (long long)h->ldab);
+    return cuda_fail(h, phase_reduce_to_band(h, (c128*)A_dev, lda, (c128*)band_dev, ldab, (cudaStream_t)stream), "reduce_to_band");
+}
+
+int eigh_band_to_tridiag(eigh_handle_t h, void* band_dev, int64_t ldab, double* d_dev, double* e_dev, void* stream) {
+    int rc = ensure_ready(h);
+    if (rc) return rc;
+    if (!band_dev) return -2;
+    if (ldab < h->ldab) return set_err(h, -3, "ldab must be >= %lld", (long long)h->ldab);
+    if (!d_dev) return -4;
+    if (!e_dev && h->N > 1) return -5;
+    return cuda_fail(h, phase_band_to_tridiag(h, (c128*)band_dev, ldab, d_dev, e_dev, (cudaStream_t)stream), "band_to_tridiag");
+}
+
+int eigh_tridiag_dc(eigh_handle_t h, const double* d_dev, const double* e_dev, double* W_dev, double* Q_dev,
+                    int64_t ldq, void* stream) {
+    int rc = ensure_ready(h);
+    if (rc) return rc;
+    if (!d_dev) return -2;
+    if (!e_dev && h->N > 1) return -3;
+    if (!W_dev) return -4;
+    if (!Q_dev) return -5;
+    if (ldq < h->N) return -6;
+    int nfail = 0;
+    rc = phase_tridiag_dc(h, d_dev, e_dev, W_dev, Q_dev, ldq, (cudaStream_t)stream, &nfail);
+    if (rc) return cuda_fail(h, rc, "tridiag_dc");
+    if (nfail) set_err(h, nfail, "%d secular roots did not converge", nfail);
+    return nfail;
+}
+
+int eigh_backtransform_band(eigh_handle_t h, const double* Q_dev, int64_t ldq, void* Z_dev, int64_t ldz, void* stream) {
+    int rc = ensure_ready(h);
+    if (rc) return rc;
+    if (!Q_dev) return -2;
+    if (ldq < h->N) return -3;
+    if (!Z_dev) return -4;
+    if (ldz < h->N) return -5;
+    return cuda_fail(h, phase_backtransform_band(h, Q_dev, ldq, (c128*)Z_dev, ldz, (cudaStream_t)stream), "backtransform_band");
+}
+
+int eigh_backtransform_full(eigh_handle_t h, const void* A_dev, int64_t lda, void* Z_dev, int64_t ldz, void* stream) {
+    int rc = ensure_ready(h);
+    if (rc) return rc;
+    if (!A_dev) return -2;
+    if (lda < h->N) return -3;
+    if (!Z_dev) return -4;
+    if (ldz < h->N) return -5;
+    return cuda_fail(h, phase_backtransform_full(h, (const c128*)A_dev, lda, (c128*)Z_dev, ldz, (cudaStream_t)stream), "backtransform_full");
+}
+
+int eigh_solve(eigh_handle_t h, void* A_dev, int64_t lda, double* W_dev, void* Z_dev, void* stream) {
+    int rc = ensure_ready(h);
+    if (rc) return rc;
+    if (!A_dev) return -2;
+    if (lda < h->N) return -3;
+    if (!W_dev) return -4;
+    if (!Z_dev) return -5;
+    cudaStream_t s = (cudaStream_t)stream;
+    const WsPlan& p = h->plan;
+    c128* band = ws_ptr<c128>(h, p.band);
+    double* d = ws_ptr<double>(h, p.d);
+    double* e = ws_ptr<double>(h, p.e);
+    double* Qt = ws_ptr<double>(h, p.Qt);
+    const int64_t ldq = round_up(h->N, 8);
+    h->launches = 0;
+    int nfail = 0;
+    cudaEventRecord(h->ev[0], s);
+    rc = phase_reduce_to_band(h, (c128*)A_dev, lda, band, h->ldab, s);
+    if (rc) return cuda_fail(h, rc, "reduce_to_band");
+    cudaEventRecord(h->ev[1], s);
+    rc = phase_band_to_tridiag(h, band, h->ldab, d, e, s);
+    if (rc) return cuda_fail(h, rc, "band_to_tridiag");
+    cudaEventRecord(h->ev[2], s);
+    rc = phase_tridiag_dc(h, d, e, W_dev, Qt, ldq, s, &nfail);
+    if (rc) return cuda_fail(h, rc, "tridiag_dc");
+    cudaEventRecord(h->ev[3], s);
+    rc = phase_backtransform_band(h, Qt, ldq, (c128*)Z_dev, h->N, s);
+    if (rc) return cuda_fail(h, rc, "backtransform_band");
+    cudaEventRecord(h->ev[4], s);
+    rc = phase_backtransform_full(h, (const c128*)A_dev, lda, (c128*)Z_dev, h->N, s);
+    if (rc) return cuda_fail(h, rc, "backtransform_full");
+    cudaEventRecord(h->ev[5], s);
+    cudaError_t ce = cudaStreamSynchronize(s);
+    if (ce != cudaSuccess) return set_err(h, 1000 + (int)ce, "eigh_solve: %s", cudaGetErrorString(ce));
+    for (int i = 0; i < 5; ++i) {
+        float ms = 0.f;
+        cudaEventElapsedTime(&ms, h->ev[i], h->ev[i + 1]);
+        h->phase_ms[i] = ms;
+    }
+    if (nfail) set_err(h, nfail, "%d secular roots did not converge", nfail);
+    return nfail;
+}
+
+int eigh_phase_times(eigh_handle_t h, double ms[5]) {
+    if (!h) return -1;
+    if (!ms) return -2;
+    for (int i = 0; i < 5; ++i) ms[i] = h->phase_ms[i];
+    return 0;
+}
+
+int64_t eigh_launch_count(eigh_handle_t h) { return h ? h->launches : -1; }
+
+const char* eigh_last_error(eigh_handle_t h) { return h ? h->err : "null handle"; }
+
+int eigh_destroy(eigh_handle_t h) {
+    if (!h) return -1;
+    if (h->events_ok)
+        for (int i = 0; i < 6; ++i) cudaEventDestroy(h->ev[i]);
+    delete h;
+    return 0;
+}
+
+// ------------------------------------------------------------------------- kernel-level entries
+int eigh_k_zgemm(eigh_handle_t h, char opA, char opB, int64_t M, int64_t N, int64_t K, double alpha,
+                 const void* A_dev, int64_t lda, const void* B_dev, int64_t ldb, int64_t K2, const void* A2_dev,
+                 int64_t lda2, const void* B2_dev, int64_t ldb2, double beta, void* C_dev, int64_t ldc,
+                 int lower_only, int splitk, void* stream) {
+    int rc = ensure_ready(h);
+    if (rc) return rc;
+    const bool ta = (opA == 'C' || opA == 'c'), tb = (opB == 'C' || opB == 'c');
+    if (!ta && opA != 'N' && opA != 'n') return -2;
+    if (!tb && opB != 'N' && opB != 'n') return -3;
+    if (ta && tb) return set_err(h, -3, "opA = opB = 'C' is not instantiated");
+    if (M < 0 || N < 0 || K < 0) return -4;
+    if (splitk < 1) return -20;
+    ZgemmArgs a;
+    memset(&a, 0, sizeof(a));
+    a.M = (int)M; a.N = (int)N; a.K1 = (int)K; a.K2 = (int)K2;
+    a.A1 = (const c128*)A_dev; a.B1 = (const c128*)B_dev; a.lda1 = lda; a.ldb1 = ldb;
+    a.A2 = (const c128*)A2_dev; a.B2 = (const c128*)B2_dev; a.lda2 = lda2; a.ldb2 = ldb2;
+    a.C = (c128*)C_dev; a.ldc = ldc; a.alpha = alpha; a.beta = beta;
+    a.lower_only = lower_only & 1; a.splitk = splitk;
+    a.partial = ws_ptr<c128>(h, h->plan.gemm_partial);
+    if (splitk > 1 && (size_t)splitk * M * N * sizeof(c128) > h->plan.gemm_partial_bytes)
+        return set_err(h, -20, "splitk partials exceed workspace");
+    const bool small_tile = (M <= 64) || (lower_only & 2);
+    rc = zgemm_launch(a, ta, tb, ZMODE_GEMM, small_tile, (cudaStream_t)stream, &h->launches);
+    return rc ? cuda_fail(h, 1000 + rc, "zgemm") : 0;
+}
+
+int eigh_k_zhemm_lower(eigh_handle_t h, int64_t M, int64_t N, const void* A_dev, int64_t lda, const void* B_dev,
+                       int64_t ldb, void* C_dev, int64_t ldc, int splitk, void* stream) {
+    int rc = ensure_ready(h);
+    if (rc) return rc;
+    if (M < 0 || N < 0) return -2;
+    if (splitk < 1) return -10;
+    ZgemmArgs a;
+    memset(&a, 0, sizeof(a));
+    a.M = (int)M; a.N = (int)N; a.K1 = (int)M;
+    a.A1 = (const c128*)A_dev; a.B1 = (const c128*)B_dev; a.lda1 = lda; a.ldb1 = ldb;
+    a.C = (c128*)C_dev; a.ldc = ldc; a.alpha = 1.0; a.beta = 0.0; a.splitk = splitk;
+    a.partial = ws_ptr<c128>(h, h->plan.gemm_partial);
+    if (splitk > 1 && (size_t)splitk * M * N * sizeof(c128) > h->plan.gemm_partial_bytes)
+        return set_err(h, -10, "splitk partials exceed workspace");
+    rc = zgemm_launch(a, false, false, ZMODE_HEMM, true, (cudaStream_t)stream, &h->launches);
+    return rc ? cuda_fail(h, 1000 + rc, "zhemm") : 0;
+}
+
+int eigh_k_dgemm(eigh_handle_t h, int64_t M, int64_t N, int64_t K, const double* A_dev, int64_t lda,
+                 const int32_t* a_col_idx_dev, const double* B_dev, int64_t ldb, double* C_dev, int64_t ldc,
+                 void* stream) {
+    int rc = ensure_ready(h);
+    if (rc) return rc;
+    if (M < 0 || N < 0 || K < 0) return -2;
+    if ((lda & 1) || (ldb & 1) || ((uintptr_t)A_dev & 15) || ((uintptr_t)B_dev & 15))
+        return set_err(h, -6, "dgemm needs 16-byte aligned A, B and even lda, ldb");
+    DgemmArgs a;
+    memset(&a, 0, sizeof(a));
+    a.A = A_dev; a.lda = lda; a.B = B_dev; a.ldb = ldb; a.C = C_dev; a.ldc = ldc;
+    a.a_col_idx = a_col_idx_dev; a.desc = nullptr;
+    a.one.M = (int)M; a.one.N = (int)N; a.one.K = (int)K;
+    rc = dgemm_launch_desc(a, 1, (int)M, (int)N, (cudaStream_t)stream, &h->launches);
+    return rc ? cuda_fail(h, 1000 + rc, "dgemm") : 0;
+}
+
+}  // extern "C"
+
+// ------------------------------------------------------------------------- FP64 peak microbenchmarks
+namespace eigh {
+__global__ void __launch_bounds__(256) peak_dmma_kernel(int64_t iters, double* sink) {
+    double c[16][2];
+#pragma unroll
+    for (int i = 0; i < 16; ++i) { c[i][0] = 0.0; c[i][1] = 0.0; }
+    const double a = 1.0 + 1e-9 * threadIdx.x, b = 1.0 - 1e-9 * threadIdx.x;
+    for (int64_t it = 0; it < iters; ++it) {
+#pragma unroll
+        for (int i = 0; i < 16; ++i) dmma884(c[i][0], c[i][1], a, b);
+    }
+    double s = 0.0;
+#pragma unroll
+    for (int i = 0; i < 16; ++i) s += c[i][0] + c[i][1];
+    if (s == 123.456) sink[0] = s;
+}
+__global__ void __launch_bounds__(256) peak_dfma_kernel(int64_t iters, double* sink) {
+    double c[16];
+#pragma unroll
+    for (int i = 0; i < 16; ++i) c[i] = 1e-3 * i;
+    const double a = 1.0 + 1e-9 * threadIdx.x, b = 1e-9 * threadIdx.x;
+    for (int64_t it = 0; it < iters; ++it) {
+#pragma unroll
+        for (int i = 0; i < 16; ++i) c[i] = fma(c[i], a, b);
+    }
+    double s = 0.0;
+#pragma unroll
+    for (int i = 0; i < 16; ++i) s += c[i];
+    if (s == 123.456) sink[0] = s;
+}
+}  // namespace eigh
+
+extern "C" int eigh_k_fp64_peak(int use_dmma, int64_t iters, double* tflops, double* ms_out, void* stream) {
+    if (iters < 1) return -2;
+    if (!tflops) return -3;
+    cudaStream_t s = (cudaStream_t)stream;
+    int dev = 0, sms = 0;
+    EIGH_CUDA_OK(cudaGetDevice(&dev));
+    EIGH_CUDA_OK(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+    double* sink = nullptr;
+    EIGH_CUDA_OK(cudaMalloc(&sink, 8));
+    cudaEvent_t e0, e1;
+    EIGH_CUDA_OK(cudaEventCreate(&e0));
+    EIGH_CUDA_OK(cudaEventCreate(&e1));
+    const int blocks = sms * 4, threads = 256;
+    for (int rep = 0; rep < 2; ++rep) {   // first pass = warm-up
+        EIGH_CUDA_OK(cudaEventRecord(e0, s));
+        if (use_dmma) eigh::peak_dmma_kernel<<<blocks, threads, 0, s>>>(iters, sink);
+        else eigh::peak_dfma_kernel<<<blocks, threads, 0, s>>>(iters, sink);
+        EIGH_CUDA_OK(cudaGetLastError());
+        EIGH_CUDA_OK(cudaEventRecord(e1, s));
+        EIGH_CUDA_OK(cudaEventSynchronize(e1));
+    }
+    float ms = 0.f;
+    EIGH_CUDA_OK(cudaEventElapsedTime(&ms, e0, e1));
+    const double warps = (double)blocks * threads / 32.0;
+    const double flops = use_dmma ? warps * (double)iters * 16.0 * 512.0
+                                  : (double)blocks * threads * (double)iters * 16.0 * 2.0;
+    *tflops = flops / (ms * 1e-3) / 1e12;
+    if (ms_out) *ms_out = ms;
+    cudaEventDestroy(e0);
+    cudaEventDestroy(e1);
+    cudaFree(sink);
+    return 0;
+}

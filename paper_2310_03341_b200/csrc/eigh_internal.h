@@ -1,0 +1,73 @@
+// eigh_internal.h -- handle, workspace plan and phase drivers (host side) of b200-eigh.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include <stdio.h>
+#include <string.h>
+
+#include "../../include/eigh.h"
+#include "common.cuh"
+
+namespace eigh {
+
+// Byte offsets of the regions inside the caller-provided workspace (all 256-byte aligned).
+struct WsPlan {
+    size_t gemm_partial, gemm_partial_bytes;   // split-K partial sums
+    size_t band;                               // ldab x N c128 band storage
+    size_t tau1;                               // N c128: stage-1 taus
+    size_t T1;                                 // npanels x b x b c128: stage-1 compact-WY T factors
+    size_t Vp, VT, X;                          // (N x b) c128 panel temporaries (Vp = explicit V)
+    size_t small;                              // b x b c128 scratch (Gram, S) x 4
+    size_t panel_sync;                         // cooperative panel kernel: counters + partial dots
+    size_t V2;                                 // packed stage-2 reflectors, N(N-1)/2 c128
+    size_t bc_progress;                        // bulge chasing progress counters (N int32)
+    size_t d, e, sgn;                          // tridiagonal (N doubles each) and row signs
+    size_t dc;                                 // D&C arena
+    size_t dc_bytes;
+    size_t Qt;                                 // D&C result N x nev real (lives inside dc arena)
+    size_t bt;                                 // back-transform scratch (diamond V/T buffers, Y)
+    size_t bt_bytes;
+    size_t total;
+};
+
+}  // namespace eigh
+
+struct eigh_handle_s {
+    int64_t N, nev;
+    int b;          // band width
+    int g;          // WY group size for S4a
+    int leaf;       // D&C leaf size
+    int p4b_merge;  // panels per WY block in S4b
+    int64_t ldab;   // band storage leading dimension
+    void* ws;
+    size_t ws_bytes;
+    eigh::WsPlan plan;
+    bool planned;
+    char err[512];
+    double phase_ms[5];
+    int64_t launches;
+    cudaEvent_t ev[6];
+    bool events_ok;
+    int num_sms;
+};
+
+namespace eigh {
+
+void plan_workspace(eigh_handle_s* h);
+template <typename T>
+static inline T* ws_ptr(eigh_handle_s* h, size_t off) { return reinterpret_cast<T*>((char*)h->ws + off); }
+
+int set_err(eigh_handle_s* h, int code, const char* fmt, ...);
+
+// phase drivers (each enqueues on `s`; returns 0 or an error code)
+int phase_reduce_to_band(eigh_handle_s* h, c128* A, int64_t lda, c128* band, int64_t ldab, cudaStream_t s);
+int phase_band_to_tridiag(eigh_handle_s* h, c128* band, int64_t ldab, double* d, double* e, cudaStream_t s);
+int phase_tridiag_dc(eigh_handle_s* h, const double* d, const double* e, double* W, double* Q, int64_t ldq,
+                     cudaStream_t s, int* nfail);
+int phase_backtransform_band(eigh_handle_s* h, const double* Q, int64_t ldq, c128* Z, int64_t ldz,
+                             cudaStream_t s);
+int phase_backtransform_full(eigh_handle_s* h, const c128* A, int64_t lda, c128* Z, int64_t ldz,
+                             cudaStream_t s);
+
+
+}  // namespace eigh

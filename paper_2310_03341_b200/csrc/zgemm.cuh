@@ -1,0 +1,277 @@
+// zgemm.cuh -- complex-FP64 GEMM engine on the FP64 tensor-core path (mma.sync m8n8k4 -> DMMA.8x8x4).
+//
+//   C <- alpha * opA(A1) opB(B1) [+ alpha * opA(A2) opB(B2)] + beta * C            (ZMODE_GEMM)
+//   C <- Herm(A1) * B1,  A1 Hermitian with only the lower triangle + 64-aligned diagonal
+//        blocks valid                                                                (ZMODE_HEMM)
+//
+// Used by S1 (V^H V, V T, HEMM-lower, V^H X, W, HER2K-lower) and S4b (WY application),
+// SURVEY.md 8(a) rows S1.2-S1.5, S4b.  One complex MAC = 4 real DMMAs on (re, im) fragments;
+// conjugation is folded into fragment sign flips.  Tiles are staged global -> shared with a
+// 4-stage cp.async (LDGSTS) pipeline; shared-memory strides are padded so that every 128-bit
+// fragment load of a quarter warp hits 8 distinct 16-byte bank groups.
+#pragma once
+#include "common.cuh"
+
+namespace eigh {
+
+struct ZgemmArgs {
+    int M, N;
+    int K1, K2;                       // inner lengths of pair 1 and (optional) pair 2
+    const c128 *A1, *B1, *A2, *B2;
+    int64_t lda1, ldb1, lda2, ldb2;
+    c128* C;
+    int64_t ldc;
+    double alpha, beta;
+    int lower_only;                   // skip tiles strictly above the diagonal
+    int splitk;                       // >= 1
+    c128* partial;                    // [splitk][N][M] raw accumulators when splitk > 1
+};
+
+enum { ZMODE_GEMM = 0, ZMODE_HEMM = 1 };
+
+constexpr int ZG_BK = 8;
+constexpr int ZG_STAGES = 4;
+constexpr int ZG_KSTRIDE = ZG_BK + 4;   // K-contiguous tiles: stride == 4 (mod 8) 16B-units
+
+template <int WARPS_M, int WARPS_N, bool TA, bool TB, int MODE>
+struct ZgemmCfg {
+    static constexpr int BM = 32 * WARPS_M, BN = 32 * WARPS_N, NT = 32 * WARPS_M * WARPS_N;
+    static constexpr int SA_N = BM + 2;                       // M-contiguous A tile: As[k][m]
+    static constexpr int SB_C = BN + 2;                       // N-contiguous B tile: Bs[k][n]
+    static constexpr int A_N_SIZE = ZG_BK * SA_N, A_C_SIZE = BM * ZG_KSTRIDE;
+    static constexpr int A_STAGE = (MODE == ZMODE_HEMM) ? (A_N_SIZE > A_C_SIZE ? A_N_SIZE : A_C_SIZE)
+                                                         : (TA ? A_C_SIZE : A_N_SIZE);
+    static constexpr int B_STAGE = TB ? ZG_BK * SB_C : BN * ZG_KSTRIDE;
+    static constexpr int STAGE = A_STAGE + B_STAGE;
+    static constexpr size_t SMEM_BYTES = (size_t)ZG_STAGES * STAGE * sizeof(c128);
+};
+
+// One k-step (4 complex k) x 2 per stage.  ACT: A tile is K-contiguous (As[m][k]); CONJA: conj(A).
+template <int BM, int BN, bool ACT, bool CONJA, bool BCT, bool CONJB>
+__device__ __forceinline__ void zgemm_compute_stage(const c128* __restrict__ As, const c128* __restrict__ Bs,
+                                                    int wm0, int wn0, int g, int t,
+                                                    double (&cr)[4][4][2], double (&ci)[4][4][2]) {
+    constexpr int SA_N = BM + 2, SB_C = BN + 2;
+#pragma unroll
+    for (int kk = 0; kk < ZG_BK; kk += 4) {
+        double ar[4], ai[4], nai[4], br[4], bi[4];
+#pragma unroll
+        for (int i = 0; i < 4; ++i) {
+            const int m = wm0 + 8 * i + g;
+            const c128 a = ACT ? As[m * ZG_KSTRIDE + kk + t] : As[(kk + t) * SA_N + m];
+            ar[i] = a.x;
+            ai[i] = CONJA ? -a.y : a.y;
+            nai[i] = CONJA ? a.y : -a.y;
+        }
+#pragma unroll
+        for (int j = 0; j < 4; ++j) {
+            const int n = wn0 + 8 * j + g;
+            const c128 b = BCT ? Bs[(kk + t) * SB_C + n] : Bs[n * ZG_KSTRIDE + kk + t];
+            br[j] = b.x;
+            bi[j] = CONJB ? -b.y : b.y;
+        }
+#pragma unroll
+        for (int i = 0; i < 4; ++i)
+#pragma unroll
+            for (int j = 0; j < 4; ++j) dmma884(cr[i][j][0], cr[i][j][1], ar[i], br[j]);
+#pragma unroll
+        for (int i = 0; i < 4; ++i)
+#pragma unroll
+            for (int j = 0; j < 4; ++j) dmma884(ci[i][j][0], ci[i][j][1], ar[i], bi[j]);
+#pragma unroll
+        for (int i = 0; i < 4; ++i)
+#pragma unroll
+            for (int j = 0; j < 4; ++j) dmma884(cr[i][j][0], cr[i][j][1], nai[i], bi[j]);
+#pragma unroll
+        for (int i = 0; i < 4; ++i)
+#pragma unroll
+            for (int j = 0; j < 4; ++j) dmma884(ci[i][j][0], ci[i][j][1], ai[i], br[j]);
+    }
+}
+
+template <int WARPS_M, int WARPS_N, bool TA, bool TB, int MODE, int MINB>
+__global__ void __launch_bounds__(32 * WARPS_M * WARPS_N, MINB) zgemm_kernel(const ZgemmArgs p) {
+    using Cfg = ZgemmCfg<WARPS_M, WARPS_N, TA, TB, MODE>;
+    constexpr int BM = Cfg::BM, BN = Cfg::BN, NT = Cfg::NT, BK = ZG_BK;
+    extern __shared__ __align__(16) unsigned char zg_smem_raw[];
+    c128* smem = reinterpret_cast<c128*>(zg_smem_raw);
+
+    const int m0 = blockIdx.x * BM, n0 = blockIdx.y * BN;
+    if (p.lower_only && m0 + BM - 1 < n0) return;
+
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int g = lane >> 2, t = lane & 3;
+    const int wm0 = (warp % WARPS_M) * 32, wn0 = (warp / WARPS_M) * 32;
+
+    const int nkb1 = (p.K1 + BK - 1) / BK;
+    const int nkb2 = (p.A2 != nullptr) ? (p.K2 + BK - 1) / BK : 0;
+    const int nkb = nkb1 + nkb2;
+    const int per = (nkb + p.splitk - 1) / p.splitk;
+    const int kb_begin = blockIdx.z * per;
+    const int kb_end = min(nkb, kb_begin + per);
+
+    double cr[4][4][2], ci[4][4][2];
+#pragma unroll
+    for (int i = 0; i < 4; ++i)
+#pragma unroll
+        for (int j = 0; j < 4; ++j) cr[i][j][0] = cr[i][j][1] = ci[i][j][0] = ci[i][j][1] = 0.0;
+
+    auto a_ctype = [&](int kb) -> bool {
+        if (MODE == ZMODE_HEMM) return kb * BK >= m0 + BM;
+        return TA;
+    };
+
+    auto load_stage = [&](int stage, int kb) {
+        c128* As = smem + (size_t)stage * Cfg::STAGE;
+        c128* Bs = As + Cfg::A_STAGE;
+        const bool second = kb >= nkb1;
+        const c128* A = second ? p.A2 : p.A1;
+        const c128* B = second ? p.B2 : p.B1;
+        const int64_t lda = second ? p.lda2 : p.lda1, ldb = second ? p.ldb2 : p.ldb1;
+        const int Kp = second ? p.K2 : p.K1;
+        const int k0 = (second ? kb - nkb1 : kb) * BK;
+        if (!a_ctype(kb)) {
+            // A element (m,k) at A[m + k*lda], M-contiguous
+#pragma unroll
+            for (int it = 0; it < BM * BK / NT; ++it) {
+                const int idx = tid + it * NT;
+                const int m = idx % BM, k = idx / BM;
+                const int gm = m0 + m, gk = k0 + k;
+                const bool ok = gm < p.M && gk < Kp;
+                const c128* src = ok ? A + gm + (int64_t)gk * lda : A;
+                cp_async16(As + k * Cfg::SA_N + m, src, ok ? 16 : 0);
+            }
+        } else {
+            // A element (m,k) = conj(A[k + m*lda]), K-contiguous
+#pragma unroll
+            for (int it = 0; it < BM * BK / NT; ++it) {
+                const int idx = tid + it * NT;
+                const int k = idx % BK, m = idx / BK;
+                const int gm = m0 + m, gk = k0 + k;
+                const bool ok = gm < p.M && gk < Kp;
+                const c128* src = ok ? A + gk + (int64_t)gm * lda : A;
+                cp_async16(As + m * ZG_KSTRIDE + k, src, ok ? 16 : 0);
+            }
+        }
+        if (!TB) {
+            // B element (k,n) at B[k + n*ldb], K-contiguous
+#pragma unroll
+            for (int it = 0; it < BN * BK / NT; ++it) {
+                const int idx = tid + it * NT;
+                const int k = idx % BK, n = idx / BK;
+                const int gn = n0 + n, gk = k0 + k;
+                const bool ok = gn < p.N && gk < Kp;
+                const c128* src = ok ? B + gk + (int64_t)gn * ldb : B;
+                cp_async16(Bs + n * ZG_KSTRIDE + k, src, ok ? 16 : 0);
+            }
+        } else {
+            // B element (k,n) = conj(B[n + k*ldb]), N-contiguous
+#pragma unroll
+            for (int it = 0; it < BN * BK / NT; ++it) {
+                const int idx = tid + it * NT;
+                const int n = idx % BN, k = idx / BN;
+                const int gn = n0 + n, gk = k0 + k;
+                const bool ok = gn < p.N && gk < Kp;
+                const c128* src = ok ? B + gn + (int64_t)gk * ldb : B;
+                cp_async16(Bs + k * Cfg::SB_C + n, src, ok ? 16 : 0);
+            }
+        }
+    };
+
+    // prologue
+#pragma unroll
+    for (int s = 0; s < ZG_STAGES - 1; ++s) {
+        if (kb_begin + s < kb_end) load_stage(s, kb_begin + s);
+        cp_async_commit();
+    }
+    for (int kb = kb_begin; kb < kb_end; ++kb) {
+        cp_async_wait<ZG_STAGES - 2>();
+        __syncthreads();
+        {
+            const int nxt = kb + ZG_STAGES - 1;
+            if (nxt < kb_end) load_stage((nxt - kb_begin) % ZG_STAGES, nxt);
+            cp_async_commit();
+        }
+        const int stage = (kb - kb_begin) % ZG_STAGES;
+        const c128* As = smem + (size_t)stage * Cfg::STAGE;
+        const c128* Bs = As + Cfg::A_STAGE;
+        if (MODE == ZMODE_HEMM) {
+            if (a_ctype(kb))
+                zgemm_compute_stage<BM, BN, true, true, TB, TB>(As, Bs, wm0, wn0, g, t, cr, ci);
+            else
+                zgemm_compute_stage<BM, BN, false, false, TB, TB>(As, Bs, wm0, wn0, g, t, cr, ci);
+        } else {
+            zgemm_compute_stage<BM, BN, TA, TA, TB, TB>(As, Bs, wm0, wn0, g, t, cr, ci);
+        }
+    }
+    cp_async_wait<0>();
+
+    // epilogue
+    if (p.splitk > 1) {
+        c128* P = p.partial + (size_t)blockIdx.z * p.M * p.N;
+#pragma unroll
+        for (int i = 0; i < 4; ++i) {
+            const int row = m0 + wm0 + 8 * i + g;
+#pragma unroll
+            for (int j = 0; j < 4; ++j)
+#pragma unroll
+                for (int e = 0; e < 2; ++e) {
+                    const int col = n0 + wn0 + 8 * j + 2 * t + e;
+                    if (row < p.M && col < p.N) P[row + (size_t)col * p.M] = cmake(cr[i][j][e], ci[i][j][e]);
+                }
+        }
+    } else {
+        const double alpha = p.alpha, beta = p.beta;
+#pragma unroll
+        for (int i = 0; i < 4; ++i) {
+            const int row = m0 + wm0 + 8 * i + g;
+#pragma unroll
+            for (int j = 0; j < 4; ++j)
+#pragma unroll
+                for (int e = 0; e < 2; ++e) {
+                    const int col = n0 + wn0 + 8 * j + 2 * t + e;
+                    if (row < p.M && col < p.N) {
+                        c128* dst = p.C + row + (int64_t)col * p.ldc;
+                        c128 v = cmake(alpha * cr[i][j][e], alpha * ci[i][j][e]);
+                        if (beta != 0.0) {
+                            const c128 o = *dst;
+                            v.x = fma(beta, o.x, v.x);
+                            v.y = fma(beta, o.y, v.y);
+                        }
+                        *dst = v;
+                    }
+                }
+        }
+    }
+}
+
+// C = alpha * sum_s partial[s] + beta * C   (deterministic order s = 0..splitk-1)
+static __global__ void zgemm_splitk_reduce_kernel(int M, int N, int splitk, const c128* __restrict__ partial,
+                                           double alpha, double beta, c128* __restrict__ C, int64_t ldc,
+                                           int lower_only_tiles, int BM, int BN) {
+    const int64_t total = (int64_t)M * N;
+    for (int64_t idx = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; idx < total;
+         idx += (int64_t)gridDim.x * blockDim.x) {
+        const int row = (int)(idx % M), col = (int)(idx / M);
+        if (lower_only_tiles) {
+            const int m0 = (row / BM) * BM, n0 = (col / BN) * BN;
+            if (m0 + BM - 1 < n0) continue;
+        }
+        double sx = 0.0, sy = 0.0;
+        for (int s = 0; s < splitk; ++s) {
+            const c128 v = partial[(size_t)s * total + idx];
+            sx += v.x; sy += v.y;
+        }
+        c128* dst = C + row + (int64_t)col * ldc;
+        c128 v = cmake(alpha * sx, alpha * sy);
+        if (beta != 0.0) { const c128 o = *dst; v.x = fma(beta, o.x, v.x); v.y = fma(beta, o.y, v.y); }
+        *dst = v;
+    }
+}
+
+// Host launcher (zgemm.cu).  small_tile: 64x64 tiles (4 warps) instead of 128x64 (8 warps).
+// Returns a cudaError_t as int (0 = ok).  `launches` (optional) is incremented per kernel launch.
+int zgemm_launch(const ZgemmArgs& a, bool ta, bool tb, int mode, bool small_tile, cudaStream_t stream,
+                 int64_t* launches);
+
+}  // namespace eigh
