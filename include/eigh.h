@@ -63,6 +63,14 @@ int eigh_set_workspace(eigh_handle_t h, void* ws_dev, size_t bytes);
 int eigh_solve(eigh_handle_t h, void* A_dev, int64_t lda, double* W_dev, void* Z_dev,
                void* stream);
 
+/* The same solve with HOST buffers (end-to-end path): copies A_host (N x N c128, lda >= N,
+ * pinned or pageable) to A_scratch_dev, runs eigh_solve, copies W (N doubles) and Z (N x nev
+ * c128) back to W_host / Z_host.  A_scratch_dev (lda*N c128), W_scratch_dev (N doubles) and
+ * Z_scratch_dev (N*nev c128) are caller-owned device buffers.  A_host is not modified.
+ * Synchronises `stream` before returning. */
+int eigh_solve_host(eigh_handle_t h, const void* A_host, int64_t lda, double* W_host, void* Z_host,
+                    void* A_scratch_dev, double* W_scratch_dev, void* Z_scratch_dev, void* stream);
+
 /* Per-phase device times of the last eigh_solve, in ms, from CUDA events on the solve's
  * stream: ms[0] = full->band, [1] = band->tridiagonal, [2] = tridiagonal D&C,
  * [3] = band back-transform, [4] = full back-transform. */

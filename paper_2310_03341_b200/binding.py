@@ -24,6 +24,7 @@ SIGNATURES = {
     "eigh_workspace_size": (_sz, [_vp]),
     "eigh_set_workspace": (_int, [_vp, _vp, _sz]),
     "eigh_solve": (_int, [_vp, _vp, _i64, _vp, _vp, _vp]),
+    "eigh_solve_host": (_int, [_vp, _vp, _i64, _vp, _vp, _vp, _vp, _vp, _vp]),
     "eigh_phase_times": (_int, [_vp, _dp]),
     "eigh_launch_count": (_i64, [_vp]),
     "eigh_last_error": (ctypes.c_char_p, [_vp]),
@@ -133,6 +134,14 @@ class Eigh:
         rc = self.lib.eigh_solve(self.h, _ptr(At), self.N, _ptr(W), _ptr(Zt), _stream())
         self._check(rc, "eigh_solve")
         return W, Zt
+
+    def solve_host(self, At_host, W_host, Zt_host, At_dev, W_dev, Zt_dev):
+        """eigh_solve_host: host tensors in/out (pinned for speed), device scratch supplied by the
+        caller.  At_host is not modified."""
+        rc = self.lib.eigh_solve_host(self.h, _ptr(At_host), self.N, _ptr(W_host), _ptr(Zt_host),
+                                      _ptr(At_dev), _ptr(W_dev), _ptr(Zt_dev), _stream())
+        self._check(rc, "eigh_solve_host")
+        return W_host, Zt_host
 
     def phase_times_ms(self):
         ms = (ctypes.c_double * 5)()

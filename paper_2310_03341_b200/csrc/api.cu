@@ -27,6 +27,7 @@ static size_t bump(size_t& off, size_t bytes) {
 }
 
 size_t dc_arena_bytes(int64_t N);   // tridiag_dc.cu
+size_t dc_result_offset(int64_t N);
 size_t bt_scratch_bytes(const eigh_handle_s* h);   // backtransform.cu
 
 void plan_workspace(eigh_handle_s* h) {
@@ -52,7 +53,7 @@ void plan_workspace(eigh_handle_s* h) {
     p.sgn = bump(off, (size_t)N * sizeof(double));
     p.dc_bytes = dc_arena_bytes(N);
     p.dc = bump(off, p.dc_bytes);
-    p.Qt = p.dc;   // the D&C driver leaves its result at the start of the arena
+    p.Qt = p.dc + dc_result_offset(N);   // eigh_solve lets S3 write its result over the dead U buffer
     // back-transform scratch aliases the tail of the D&C arena (U and the dead Q buffer)
     p.bt_bytes = bt_scratch_bytes(h);
     p.bt = bump(off, p.bt_bytes);
@@ -247,6 +248,30 @@ int eigh_solve(eigh_handle_t h, void* A_dev, int64_t lda, double* W_dev, void* Z
     }
     if (nfail) set_err(h, nfail, "%d secular roots did not converge", nfail);
     return nfail;
+}
+
+int eigh_solve_host(eigh_handle_t h, const void* A_host, int64_t lda, double* W_host, void* Z_host,
+                    void* A_scratch_dev, double* W_scratch_dev, void* Z_scratch_dev, void* stream) {
+    int rc = ensure_ready(h);
+    if (rc) return rc;
+    if (!A_host) return -2;
+    if (lda < h->N) return -3;
+    if (!W_host) return -4;
+    if (!Z_host) return -5;
+    if (!A_scratch_dev) return -6;
+    if (!W_scratch_dev) return -7;
+    if (!Z_scratch_dev) return -8;
+    cudaStream_t s = (cudaStream_t)stream;
+    cudaError_t ce = cudaMemcpyAsync(A_scratch_dev, A_host, (size_t)lda * h->N * sizeof(c128), cudaMemcpyHostToDevice, s);
+    if (ce != cudaSuccess) return set_err(h, 1000 + (int)ce, "eigh_solve_host H2D: %s", cudaGetErrorString(ce));
+    rc = eigh_solve(h, A_scratch_dev, lda, W_scratch_dev, Z_scratch_dev, stream);
+    if (rc < 0 || rc >= 1000) return rc;
+    ce = cudaMemcpyAsync(W_host, W_scratch_dev, (size_t)h->N * sizeof(double), cudaMemcpyDeviceToHost, s);
+    if (ce == cudaSuccess)
+        ce = cudaMemcpyAsync(Z_host, Z_scratch_dev, (size_t)h->N * h->nev * sizeof(c128), cudaMemcpyDeviceToHost, s);
+    if (ce == cudaSuccess) ce = cudaStreamSynchronize(s);
+    if (ce != cudaSuccess) return set_err(h, 1000 + (int)ce, "eigh_solve_host D2H: %s", cudaGetErrorString(ce));
+    return rc;
 }
 
 int eigh_phase_times(eigh_handle_t h, double ms[5]) {

@@ -49,9 +49,8 @@ __global__ void __launch_bounds__(256, 1) bt_diamond_prep_kernel(const DiamondAr
     extern __shared__ __align__(16) unsigned char dp_raw[];
     const int ldv = (int)a.ldv, g = a.g;
     c128* Vs = reinterpret_cast<c128*>(dp_raw);         // ldv x g
-    c128* Gs = Vs + (size_t)ldv * g;                    // g x (g+1)
-    c128* Ts = Gs + (size_t)g * (g + 1);                // g x (g+1)
-    c128* taus = Ts + (size_t)g * (g + 1);              // g
+    c128* Gs = Vs + (size_t)ldv * g;                    // g x (g+1): strict upper = G, lower+diag = T^T
+    c128* taus = Gs + (size_t)g * (g + 1);              // g
     const int k = blockIdx.x;
     const int N = a.N, b = a.b, gs = a.gs;
     const int R0 = a.j0 + 1 + k * b;
@@ -89,18 +88,18 @@ __global__ void __launch_bounds__(256, 1) bt_diamond_prep_kernel(const DiamondAr
             const int lo = j, hi = min(ldv, i + b);
             for (int r = lo; r < hi; ++r) cfmac(s, Vs[r + i * ldv], Vs[r + j * ldv]);
         }
-        Gs[i + j * ldg] = s;
-        Ts[i + j * ldg] = cmake(0.0, 0.0);
+        if (i < j) Gs[i + j * ldg] = s;
     }
     __syncthreads();
     if (tid < g) {
         const int j = tid;
-        Ts[j + j * ldg] = taus[j];
+        // T[i,j] (i <= j) lives at Gs[j + i*ldg] (transposed into the lower triangle)
+        Gs[j + j * ldg] = taus[j];
         for (int i = j - 1; i >= 0; --i) {
             c128 s = cmake(0.0, 0.0);
-            for (int l = i + 1; l <= j; ++l) cfma(s, Gs[i + l * ldg], Ts[l + j * ldg]);
+            for (int l = i + 1; l <= j; ++l) cfma(s, Gs[i + l * ldg], Gs[j + l * ldg]);
             const c128 ti = taus[i];
-            Ts[i + j * ldg] = cmake(-(ti.x * s.x - ti.y * s.y), -(ti.x * s.y + ti.y * s.x));
+            Gs[j + i * ldg] = cmake(-(ti.x * s.x - ti.y * s.y), -(ti.x * s.y + ti.y * s.x));
         }
     }
     __syncthreads();
@@ -112,7 +111,7 @@ __global__ void __launch_bounds__(256, 1) bt_diamond_prep_kernel(const DiamondAr
         Vd[idx] = Vs[idx];
         c128 s = cmake(0.0, 0.0);
         for (int l = j; l < g; ++l) {
-            const c128 t = Ts[j + l * ldg];
+            const c128 t = Gs[l + j * ldg];        // T[j,l]
             const c128 v = Vs[rl + l * ldv];
             // v * conj(t)
             s.x += v.x * t.x + v.y * t.y;
@@ -135,7 +134,7 @@ int phase_backtransform_band(eigh_handle_s* h, const double* Qt, int64_t ldq, c1
     bt_expand_kernel<<<dim3((unsigned)ceil_div(N, 256), (unsigned)nev), 256, 0, s>>>(Qt, ldq, sgn, N, nev, Z, ldz);
     ++h->launches;
     if (N < 2) return 0;
-    const size_t smem = ((size_t)ldv * g + 2 * (size_t)g * (g + 1) + g) * sizeof(c128);
+    const size_t smem = ((size_t)ldv * g + (size_t)g * (g + 1) + g) * sizeof(c128);
     static size_t attr_smem = 0;
     if (smem > attr_smem) {
         EIGH_CUDA_OK(cudaFuncSetAttribute(bt_diamond_prep_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));

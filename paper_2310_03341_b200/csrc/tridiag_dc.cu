@@ -47,6 +47,13 @@ size_t dc_arena_bytes(int64_t N) {
     return (size_t)3 * ldq * N * sizeof(double) + dc_small_bytes(N) + 4096;
 }
 
+// offset of the U buffer inside the arena: dead once the last merge GEMM has run, so the sorted
+// N x nev result of the phase is written there (never aliases the final Q, which is QA or QB)
+size_t dc_result_offset(int64_t N) {
+    const size_t qb = ((size_t)round_up(N, 8) * N * sizeof(double) + 255) / 256 * 256;
+    return 2 * qb;
+}
+
 static DcBufs dc_carve(void* base, int64_t N) {
     DcBufs b;
     b.ldq = round_up(N, 8);
