@@ -37,11 +37,11 @@ typedef struct eigh_handle_s* eigh_handle_t;
 
 /* Plan a solve of order N returning the LOWEST nev eigenpairs (1 <= nev <= N; "all or the
  * lowest nev", PAPER.md:119-127 keeps only part of the spectrum).  No device allocation.
- * Defaults: band width b = 64, D&C leaf 32, WY group g = 64. */
+ * Defaults: band width b = 64, D&C leaf 32, WY group g = 8. */
 int eigh_create(eigh_handle_t* h, int64_t N, int64_t nev);
 
 /* Tuning knobs; must be called before eigh_workspace_size.  Keys: "band_width" (64 or 128),
- * "wy_group" (16..64, <= band_width), "dc_leaf" (8..32), "p4b_merge" (1..4 panels per WY block).
+ * "wy_group" (reflectors per compact-WY block of S4a: 8, 16 or 32), "dc_leaf" (8..32), "p4b_merge" (1..4 panels per WY block).
  * Returns -2 for an unknown key, -3 for a bad value. */
 int eigh_set_option(eigh_handle_t h, const char* key, int64_t value);
 

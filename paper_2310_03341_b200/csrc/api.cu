@@ -2,6 +2,7 @@
 #include <stdarg.h>
 #include <stdlib.h>
 
+#include <algorithm>
 #include <new>
 
 #include "dgemm.cuh"
@@ -28,7 +29,8 @@ static size_t bump(size_t& off, size_t bytes) {
 
 size_t dc_arena_bytes(int64_t N);   // tridiag_dc.cu
 size_t dc_result_offset(int64_t N);
-size_t bt_scratch_bytes(const eigh_handle_s* h);   // backtransform.cu
+size_t bt_scratch_bytes(const eigh_handle_s* h);   // bt_band.cu
+size_t bt_tneg_bytes(int64_t N);
 
 void plan_workspace(eigh_handle_s* h) {
     WsPlan& p = h->plan;
@@ -47,12 +49,16 @@ void plan_workspace(eigh_handle_s* h) {
     p.small = bump(off, (size_t)4 * b * b * sizeof(c128));
     p.panel_sync = bump(off, (size_t)(256 + 2 * 160 * (2 * b + 8) * sizeof(c128)));
     p.V2 = bump(off, (size_t)(N * (N - 1) / 2 + 2 * b) * sizeof(c128));
+    p.tau2 = bump(off, (size_t)N * bc_kmax(h) * sizeof(c128));
     p.bc_progress = bump(off, (size_t)(N + 8) * sizeof(int));
     p.d = bump(off, (size_t)N * sizeof(double));
     p.e = bump(off, (size_t)N * sizeof(double));
     p.sgn = bump(off, (size_t)N * sizeof(double));
     p.dc_bytes = dc_arena_bytes(N);
     p.dc = bump(off, p.dc_bytes);
+    // S4a keeps its T factors in the first two (dead by then) Q buffers of the D&C arena when they fit
+    if (bt_tneg_bytes(N) <= dc_result_offset(N)) p.btT = p.dc;
+    else p.btT = bump(off, bt_tneg_bytes(N));
     p.Qt = p.dc + dc_result_offset(N);   // eigh_solve lets S3 write its result over the dead U buffer
     // back-transform scratch aliases the tail of the D&C arena (U and the dead Q buffer)
     p.bt_bytes = bt_scratch_bytes(h);
@@ -78,7 +84,7 @@ int eigh_create(eigh_handle_t* out, int64_t N, int64_t nev) {
     h->N = N;
     h->nev = nev;
     h->b = 64;
-    h->g = 64;
+    h->g = 8;
     h->leaf = 32;
     h->p4b_merge = 1;
     h->num_sms = 0;
@@ -93,9 +99,8 @@ int eigh_set_option(eigh_handle_t h, const char* key, int64_t value) {
     if (!strcmp(key, "band_width")) {
         if (value != 64 && value != 128) return set_err(h, -3, "band_width must be 64 or 128");
         h->b = (int)value;
-        if (h->g > h->b) h->g = h->b;
     } else if (!strcmp(key, "wy_group")) {
-        if (value < 8 || value > 64 || value > h->b || value % 8) return set_err(h, -3, "wy_group must be a multiple of 8 in [8, min(64, band_width)]");
+        if (value != 8 && value != 16 && value != 32) return set_err(h, -3, "wy_group must be 8, 16 or 32");
         h->g = (int)value;
     } else if (!strcmp(key, "dc_leaf")) {
         if (value < 4 || value > 32) return set_err(h, -3, "dc_leaf must be in [4, 32]");

@@ -14,8 +14,8 @@
 // memory, acquire/release through L2; all band reads bypass L1).  The grid is launched
 // cooperatively so that every CTA is resident (the wait chain always ends at a running sweep).
 //
-// Reflectors (LAPACK zlarfg convention, H = I - tau v v^H, v_0 = 1) are stored packed:
-// V2[off(j) + row - j - 1], off(j) = j (N-1) - j (j-1)/2, with tau in the slot of v_0.
+// Reflectors (LAPACK zlarfg convention, H = I - tau v v^H, v_0 = 1 stored explicitly) are packed:
+// V2[off(j) + row - j - 1], off(j) = j (N-1) - j (j-1)/2; tau of (sweep j, step k) at tau2[j kmax + k].
 #include <limits.h>
 
 #include "eigh_internal.h"
@@ -30,6 +30,8 @@ struct BcArgs {
     c128* band; int64_t ldab;
     int N;
     c128* V2;
+    c128* tau2;       // [N][kmax]: tau of reflector (sweep j, step k) at tau2[j*kmax + k]
+    int kmax;
     int* progress;    // [N], zero on entry
 };
 
@@ -117,7 +119,8 @@ __global__ void __launch_bounds__(BC_NT, 1) bulge_chase_kernel(const BcArgs a) {
         c128 tau = bc_make_reflector(v, v, len, red, scal, &beta);
         if (tid < len) {
             colj[1 + tid] = (tid == 0) ? cmake(beta, 0.0) : cmake(0.0, 0.0);
-            Vj[j + 1 + tid] = (tid == 0) ? tau : v[tid];
+            Vj[j + 1 + tid] = v[tid];
+            if (tid == 0) a.tau2[(int64_t)j * a.kmax] = tau;
         }
         for (int k = 0;; ++k) {
             const int r0 = j + 1 + k * BC_B;
@@ -237,7 +240,8 @@ __global__ void __launch_bounds__(BC_NT, 1) bulge_chase_kernel(const BcArgs a) {
                     a.band[(BC_B + r - cc) + (int64_t)(r0 + cc) * ldab] = e;
                 }
             }
-            if (tid < len2) Vj[r0 + BC_B + tid] = (tid == 0) ? taun : vn[tid];
+            if (tid < len2) Vj[r0 + BC_B + tid] = vn[tid];
+            if (tid == 0) a.tau2[(int64_t)j * a.kmax + k + 1] = taun;
             __syncthreads();
             if (tid == 0) {
                 __threadfence();
@@ -294,6 +298,7 @@ int phase_band_to_tridiag(eigh_handle_s* h, c128* band, int64_t ldab, double* d,
         if (G > N - 1) G = N - 1;
         BcArgs a;
         a.band = band; a.ldab = ldab; a.N = N; a.V2 = ws_ptr<c128>(h, pl.V2); a.progress = progress;
+        a.tau2 = ws_ptr<c128>(h, pl.tau2); a.kmax = (int)bc_kmax(h);
         void* kargs[] = {(void*)&a};
         EIGH_CUDA_OK(cudaLaunchCooperativeKernel((void*)bulge_chase_kernel, dim3(G), dim3(BC_NT), kargs, smem, s));
         ++h->launches;

@@ -20,12 +20,14 @@ struct WsPlan {
     size_t small;                              // b x b c128 scratch (Gram, S) x 4
     size_t panel_sync;                         // cooperative panel kernel: counters + partial dots
     size_t V2;                                 // packed stage-2 reflectors, N(N-1)/2 c128
+    size_t tau2;                               // stage-2 taus, N x kmax c128 (kmax = bc_kmax)
     size_t bc_progress;                        // bulge chasing progress counters (N int32)
     size_t d, e, sgn;                          // tridiagonal (N doubles each) and row signs
     size_t dc;                                 // D&C arena
     size_t dc_bytes;
     size_t Qt;                                 // D&C result N x nev real (lives inside dc arena)
-    size_t bt;                                 // back-transform scratch (diamond V/T buffers, Y)
+    size_t btT;                                // S4a: -T factors of all (pass, k) steps (aliases the dead D&C Q buffers)
+    size_t bt;                                 // back-transform scratch (S4b's Y, S4a's counters)
     size_t bt_bytes;
     size_t total;
 };
@@ -58,6 +60,12 @@ template <typename T>
 static inline T* ws_ptr(eigh_handle_s* h, size_t off) { return reinterpret_cast<T*>((char*)h->ws + off); }
 
 int set_err(eigh_handle_s* h, int code, const char* fmt, ...);
+
+// steps per bulge-chasing sweep (upper bound over sweeps): reflector (j, k) starts at row j+1+k*b
+static inline int64_t bc_kmax(const eigh_handle_s* h) {
+    const int64_t k = (h->N - 1 + h->b - 1) / h->b;
+    return k < 1 ? 1 : k;
+}
 
 // phase drivers (each enqueues on `s`; returns 0 or an error code)
 int phase_reduce_to_band(eigh_handle_s* h, c128* A, int64_t lda, c128* band, int64_t ldab, cudaStream_t s);
