@@ -41,7 +41,7 @@ typedef struct eigh_handle_s* eigh_handle_t;
 int eigh_create(eigh_handle_t* h, int64_t N, int64_t nev);
 
 /* Tuning knobs; must be called before eigh_workspace_size.  Keys: "band_width" (64 or 128),
- * "wy_group" (reflectors per compact-WY block of S4a: 8, 16 or 32), "dc_leaf" (8..32), "p4b_merge" (1..4 panels per WY block).
+ * "wy_group" (reflectors per compact-WY block of S4a: 8, 16 or 32), "dc_leaf" (8..32), "p4b_merge" (1..4 panels of S1 merged into one compact-WY block of S4b; default 4).
  * Returns -2 for an unknown key, -3 for a bad value. */
 int eigh_set_option(eigh_handle_t h, const char* key, int64_t value);
 
@@ -127,8 +127,8 @@ int eigh_backtransform_full(eigh_handle_t h, const void* A_dev, int64_t lda, voi
  *   C <- alpha * opA(A) * opB(B) [+ alpha * opA(A2) * opB(B2)] + beta * C
  * opX = 'N' (as stored) or 'C' (conjugate transpose).  C is M x N, inner dimension K (K2 for
  * the optional second pair; pass A2_dev = NULL to disable).  lower_only bit 0 skips output
- * tiles that lie strictly above the diagonal (HER2K-lower); bit 1 forces the 64x64 tile
- * configuration (default: 128x64, or 64x64 when M <= 64).  splitk >= 1 partitions K over
+ * tiles that lie strictly above the diagonal (HER2K-lower); bit 2 (value 4) selects the
+ * 128x64 tile configuration (default: 64x64 tiles, two thread blocks per SM).  splitk >= 1 partitions K over
  * thread blocks with a deterministic two-pass reduction (partials in the handle workspace). */
 int eigh_k_zgemm(eigh_handle_t h, char opA, char opB, int64_t M, int64_t N, int64_t K,
                  double alpha, const void* A_dev, int64_t lda, const void* B_dev, int64_t ldb,

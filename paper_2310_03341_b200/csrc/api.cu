@@ -63,6 +63,14 @@ void plan_workspace(eigh_handle_s* h) {
     // back-transform scratch aliases the tail of the D&C arena (U and the dead Q buffer)
     p.bt_bytes = bt_scratch_bytes(h);
     p.bt = bump(off, p.bt_bytes);
+    {
+        const int64_t kb = (int64_t)h->p4b_merge * b;
+        p.b4V = bump(off, (size_t)N * kb * sizeof(c128));
+        p.b4VT = bump(off, (size_t)N * kb * sizeof(c128));
+        p.b4Y = bump(off, (size_t)kb * h->nev * sizeof(c128));
+        p.b4T = bump(off, (size_t)kb * kb * sizeof(c128));
+        p.b4G = bump(off, (size_t)2 * kb * kb * sizeof(c128));
+    }
     p.total = off;
     h->planned = true;
 }
@@ -86,7 +94,7 @@ int eigh_create(eigh_handle_t* out, int64_t N, int64_t nev) {
     h->b = 64;
     h->g = 8;
     h->leaf = 32;
-    h->p4b_merge = 1;
+    h->p4b_merge = 4;
     h->num_sms = 0;
     snprintf(h->err, sizeof(h->err), "ok");
     *out = h;
@@ -322,7 +330,9 @@ int eigh_k_zgemm(eigh_handle_t h, char opA, char opB, int64_t M, int64_t N, int6
     if (splitk > 1 && (size_t)splitk * M * N * sizeof(c128) > h->plan.gemm_partial_bytes)
         return set_err(h, -20, "splitk partials exceed workspace");
     const bool small_tile = (M <= 64) || (lower_only & 2);
+    g_zgemm_big_tiles = (lower_only & 4) != 0;
     rc = zgemm_launch(a, ta, tb, ZMODE_GEMM, small_tile, (cudaStream_t)stream, &h->launches);
+    g_zgemm_big_tiles = false;
     return rc ? cuda_fail(h, 1000 + rc, "zgemm") : 0;
 }
 

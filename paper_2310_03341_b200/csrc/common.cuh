@@ -60,6 +60,13 @@ __device__ __forceinline__ void dmma884(double& c0, double& c1, double a, double
                  : "d"(a), "d"(b));
 }
 
+// the same instruction without `volatile`: a pure function of its operands, free to be scheduled
+__device__ __forceinline__ void dmma884p(double& c0, double& c1, double a, double b) {
+    asm("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};\n"
+        : "+d"(c0), "+d"(c1)
+        : "d"(a), "d"(b));
+}
+
 // ----------------------------------------------------------------------------- host-side
 #define EIGH_CUDA_OK(expr)                                                                  \
     do {                                                                                    \

@@ -29,6 +29,7 @@ struct WsPlan {
     size_t btT;                                // S4a: -T factors of all (pass, k) steps (aliases the dead D&C Q buffers)
     size_t bt;                                 // back-transform scratch (S4b's Y, S4a's counters)
     size_t bt_bytes;
+    size_t b4V, b4VT, b4Y, b4T, b4G;           // S4b merged-panel WY blocks: V, V T^H (N x kb), Y (kb x nev), T, G (kb x kb)
     size_t total;
 };
 

@@ -33,11 +33,15 @@ static int launch_inst(const ZgemmArgs& a, cudaStream_t stream, int64_t* launche
     return 0;
 }
 
+bool g_zgemm_big_tiles = false;   // test hook (eigh_k_zgemm lower_only bit 2)
+
 int zgemm_launch(const ZgemmArgs& a, bool ta, bool tb, int mode, bool small_tile, cudaStream_t stream,
                  int64_t* launches) {
     if (a.M <= 0 || a.N <= 0) return 0;
     if (mode == ZMODE_HEMM) return launch_inst<2, 2, false, false, ZMODE_HEMM, 2>(a, stream, launches);
-    if (small_tile) {
+    // 64x64 tiles with two resident CTAs per SM are the default: measured faster than 128x64 with one
+    // CTA per SM in every shape the solver uses (profiles/r01_gemm_shapes.md)
+    if (small_tile || !g_zgemm_big_tiles) {
         if (!ta && !tb) return launch_inst<2, 2, false, false, ZMODE_GEMM, 2>(a, stream, launches);
         if (!ta && tb) return launch_inst<2, 2, false, true, ZMODE_GEMM, 2>(a, stream, launches);
         if (ta && !tb) return launch_inst<2, 2, true, false, ZMODE_GEMM, 2>(a, stream, launches);

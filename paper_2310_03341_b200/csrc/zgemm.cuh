@@ -73,19 +73,19 @@ __device__ __forceinline__ void zgemm_compute_stage(const c128* __restrict__ As,
 #pragma unroll
         for (int i = 0; i < 4; ++i)
 #pragma unroll
-            for (int j = 0; j < 4; ++j) dmma884(cr[i][j][0], cr[i][j][1], ar[i], br[j]);
+            for (int j = 0; j < 4; ++j) dmma884p(cr[i][j][0], cr[i][j][1], ar[i], br[j]);
 #pragma unroll
         for (int i = 0; i < 4; ++i)
 #pragma unroll
-            for (int j = 0; j < 4; ++j) dmma884(ci[i][j][0], ci[i][j][1], ar[i], bi[j]);
+            for (int j = 0; j < 4; ++j) dmma884p(ci[i][j][0], ci[i][j][1], ar[i], bi[j]);
 #pragma unroll
         for (int i = 0; i < 4; ++i)
 #pragma unroll
-            for (int j = 0; j < 4; ++j) dmma884(cr[i][j][0], cr[i][j][1], nai[i], bi[j]);
+            for (int j = 0; j < 4; ++j) dmma884p(cr[i][j][0], cr[i][j][1], nai[i], bi[j]);
 #pragma unroll
         for (int i = 0; i < 4; ++i)
 #pragma unroll
-            for (int j = 0; j < 4; ++j) dmma884(ci[i][j][0], ci[i][j][1], ai[i], br[j]);
+            for (int j = 0; j < 4; ++j) dmma884p(ci[i][j][0], ci[i][j][1], ai[i], br[j]);
     }
 }
 
@@ -111,10 +111,31 @@ __global__ void __launch_bounds__(32 * WARPS_M * WARPS_N, MINB) zgemm_kernel(con
     const int kb_end = min(nkb, kb_begin + per);
 
     double cr[4][4][2], ci[4][4][2];
+    // beta == +-alpha: start the accumulators at (beta/alpha) C (exact), so that the read of C overlaps
+    // the pipeline prologue instead of serialising the epilogue
+    const bool preload = (p.splitk == 1) && (p.beta != 0.0) && (p.beta == p.alpha || p.beta == -p.alpha);
+    if (preload) {
+        const double sg = (p.beta == p.alpha) ? 1.0 : -1.0;
 #pragma unroll
-    for (int i = 0; i < 4; ++i)
+        for (int i = 0; i < 4; ++i) {
+            const int row = m0 + wm0 + 8 * i + g;
 #pragma unroll
-        for (int j = 0; j < 4; ++j) cr[i][j][0] = cr[i][j][1] = ci[i][j][0] = ci[i][j][1] = 0.0;
+            for (int j = 0; j < 4; ++j)
+#pragma unroll
+                for (int e = 0; e < 2; ++e) {
+                    const int col = n0 + wn0 + 8 * j + 2 * t + e;
+                    c128 v = cmake(0.0, 0.0);
+                    if (row < p.M && col < p.N) v = p.C[row + (int64_t)col * p.ldc];
+                    cr[i][j][e] = sg * v.x;
+                    ci[i][j][e] = sg * v.y;
+                }
+        }
+    } else {
+#pragma unroll
+        for (int i = 0; i < 4; ++i)
+#pragma unroll
+            for (int j = 0; j < 4; ++j) cr[i][j][0] = cr[i][j][1] = ci[i][j][0] = ci[i][j][1] = 0.0;
+    }
 
     auto a_ctype = [&](int kb) -> bool {
         if (MODE == ZMODE_HEMM) return kb * BK >= m0 + BM;
@@ -221,7 +242,7 @@ __global__ void __launch_bounds__(32 * WARPS_M * WARPS_N, MINB) zgemm_kernel(con
                 }
         }
     } else {
-        const double alpha = p.alpha, beta = p.beta;
+        const double alpha = p.alpha, beta = preload ? 0.0 : p.beta;
 #pragma unroll
         for (int i = 0; i < 4; ++i) {
             const int row = m0 + wm0 + 8 * i + g;
@@ -269,9 +290,11 @@ static __global__ void zgemm_splitk_reduce_kernel(int M, int N, int splitk, cons
     }
 }
 
-// Host launcher (zgemm.cu).  small_tile: 64x64 tiles (4 warps) instead of 128x64 (8 warps).
+// Host launcher (zgemm.cu).  Tiles are 64x64 (4 warps, 2 CTAs/SM) unless g_zgemm_big_tiles is set and
+// small_tile is false (then 128x64, 8 warps, 1 CTA/SM).
 // Returns a cudaError_t as int (0 = ok).  `launches` (optional) is incremented per kernel launch.
 int zgemm_launch(const ZgemmArgs& a, bool ta, bool tb, int mode, bool small_tile, cudaStream_t stream,
                  int64_t* launches);
+extern bool g_zgemm_big_tiles;
 
 }  // namespace eigh
