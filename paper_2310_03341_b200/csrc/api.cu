@@ -116,6 +116,9 @@ int eigh_set_option(eigh_handle_t h, const char* key, int64_t value) {
     } else if (!strcmp(key, "p4b_merge")) {
         if (value < 1 || value > 4) return set_err(h, -3, "p4b_merge must be in [1, 4]");
         h->p4b_merge = (int)value;
+    } else if (!strcmp(key, "bc_grid")) {
+        if (value < 0 || value > 4096) return set_err(h, -3, "bc_grid must be in [0, 4096]");
+        h->bc_grid = (int)value;
     } else {
         return set_err(h, -2, "unknown option '%s'", key);
     }

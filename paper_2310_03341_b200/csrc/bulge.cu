@@ -23,8 +23,10 @@
 namespace eigh {
 
 constexpr int BC_B = 64;          // band width handled by this kernel
-constexpr int BC_LD = BC_B + 1;   // padded shared-memory leading dimension
+constexpr int BC_LD = BC_B + 1;   // padded shared-memory leading dimension of the D block
 constexpr int BC_NT = 256;
+constexpr int BC_NW = BC_NT / 32;
+constexpr int BC_NC = BC_B / 4;   // columns per thread
 
 struct BcArgs {
     c128* band; int64_t ldab;
@@ -35,229 +37,336 @@ struct BcArgs {
     int* progress;    // [N], zero on entry
 };
 
-__device__ __forceinline__ double bc_block_sum(double v, double* red) {
+// Thread layout of one chase step: warp w owns rows 8w..8w+7 of a 64 x 64 block; lane = rl + 8 q
+// owns row r = 8w + rl and the 16 columns c = q + 4 i.  Row reductions (over columns) are two
+// xor-shuffles (8, 16); column reductions (over rows) are a reduce-scatter over the rl lanes
+// followed by one pass through shared memory across the 8 warps.  A quarter warp (same q, 8
+// consecutive rows) touches 128 contiguous bytes of band storage and 8 distinct shared-memory
+// bank groups of the odd-stride D tile.
+struct BcSmem {
+    c128 D[BC_B * BC_LD];        // lower triangle of D_k (cp.async target)
+    c128 zpart[BC_NW * BC_B];    // per-warp partial column sums
+    c128 vs[BC_B];               // current reflector (zero padded)
+    c128 ws[BC_B];               // w = D v
+    c128 zs[BC_B];               // conj(tau') vn^H S
+    c128 xs[BC_B];               // first column of S (the next reflector's source)
+    double red[BC_NW];
+    double red2[BC_NW];
+};
+
+__device__ __forceinline__ double bc_warp_sum(double v) {
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    __syncthreads();
-    if (lane == 0) red[warp] = v;
-    __syncthreads();
-    double s = 0.0;
+    return v;
+}
+__device__ __forceinline__ c128 bc_shfl_xor(c128 v, int m) {
+    return cmake(__shfl_xor_sync(0xffffffffu, v.x, m), __shfl_xor_sync(0xffffffffu, v.y, m));
+}
+
+// LAPACK zlarfg scalars from alpha = x_0 and xnorm2 = sum_{i>=1} |x_i|^2 (every thread evaluates them
+// redundantly: no single-thread section).  v_i = s x_i (i >= 1), v_0 = 1, H x = beta e_1.
+__device__ __forceinline__ void bc_reflector_scalars(c128 alpha, double xnorm2, c128& tau, c128& s, double& beta) {
+    tau = cmake(0.0, 0.0);
+    s = cmake(0.0, 0.0);
+    beta = alpha.x;
+    if (xnorm2 > 0.0 || alpha.y != 0.0) {
+        beta = -copysign(sqrt(alpha.x * alpha.x + alpha.y * alpha.y + xnorm2), alpha.x);
+        const double ib = 1.0 / beta;
+        tau = cmake((beta - alpha.x) * ib, -alpha.y * ib);
+        const double dr = alpha.x - beta, di = alpha.y;
+        const double iden = 1.0 / (dr * dr + di * di);
+        s = cmake(dr * iden, -di * iden);
+    }
+}
+
+// ---- inter-CTA progress protocol -------------------------------------------------------------
+// progress[j] = number of completed chase steps of sweep j (INT_MAX when the sweep is finished).
+// Writer: the compute warps issue their band stores and arrive (without blocking) at a named
+// barrier; the publisher warp completes that barrier, executes a gpu-scope release fence (which is
+// cumulative over the stores ordered before it by the barrier) and stores the counter.  Reader:
+// one thread spins with ld.acquire.gpu; the compute-group barrier that follows orders every later
+// band load (all of them bypass L1: cp.async.cg / ld.global.cg) after the acquire.
+__device__ __forceinline__ int bc_ld_acquire(const int* p) {
+    int v;
+    asm volatile("ld.acquire.gpu.global.s32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
+    return v;
+}
+__device__ __forceinline__ void bc_st_release(int* p, int v) {
+    asm volatile("fence.acq_rel.gpu;\n\tst.relaxed.gpu.global.s32 [%0], %1;" ::"l"(p), "r"(v) : "memory");
+}
+__device__ __forceinline__ void bc_poll(const int* progress, int sweep, int need) {
+    if (sweep >= 0)
+        while (bc_ld_acquire(progress + sweep) < need) {}
+}
+// named barriers: 1 = compute group (BC_NT threads); 2, 3 = hand-off to the publisher warp (alternating)
+__device__ __forceinline__ void bc_sync_compute() { asm volatile("bar.sync 1, %0;" ::"n"(BC_NT) : "memory"); }
+__device__ __forceinline__ void bc_handoff_arrive(int odd) {
+    if (odd) asm volatile("bar.arrive 3, %0;" ::"n"(BC_NT + 32) : "memory");
+    else asm volatile("bar.arrive 2, %0;" ::"n"(BC_NT + 32) : "memory");
+}
+__device__ __forceinline__ void bc_handoff_wait(int odd) {
+    if (odd) asm volatile("bar.sync 3, %0;" ::"n"(BC_NT + 32) : "memory");
+    else asm volatile("bar.sync 2, %0;" ::"n"(BC_NT + 32) : "memory");
+}
+
+struct BcStepCtx {
+    c128* band; int64_t ldab;
+    c128* Vj; c128* tau2j;
+    int r, q, rl, lane, warp, tid;
+};
+
+// LAPACK zlarfg on a vector spread over the rows (x = element r, zero for r >= len; all four q lanes of
+// a row hold it).  Returns v_r.  One compute-group barrier inside.
+__device__ __forceinline__ c128 bc_make_reflector(c128 x, const BcStepCtx& t, int len, double* red, c128* x0,
+                                                  c128& tau, double& beta) {
+    double part = (t.q == 0 && t.r >= 1 && t.r < len) ? cabs2(x) : 0.0;
+    part = bc_warp_sum(part);
+    if (t.lane == 0) red[t.warp] = part;
+    if (t.r == 0 && t.q == 0) *x0 = x;
+    bc_sync_compute();
+    double xnorm2 = 0.0;
 #pragma unroll
-    for (int w = 0; w < BC_NT / 32; ++w) s += red[w];
-    return s;
+    for (int w = 0; w < BC_NW; ++w) xnorm2 += red[w];
+    const c128 alpha = *x0;
+    c128 s;
+    bc_reflector_scalars(alpha, xnorm2, tau, s, beta);
+    c128 v = cmake(0.0, 0.0);
+    if (t.r < len) v = (t.r == 0) ? cmake(1.0, 0.0) : cmul(s, x);
+    return v;
 }
 
-// x[0..len) in xs -> v (v_0 = 1) in vs; returns tau; beta via *beta_out.  All threads call.
-__device__ __forceinline__ c128 bc_make_reflector(const c128* xs, c128* vs, int len, double* red, c128* scal,
-                                                  double* beta_out) {
-    const int tid = threadIdx.x;
-    double part = 0.0;
-    if (tid >= 1 && tid < len) part = cabs2(xs[tid]);
-    const double xnorm2 = bc_block_sum(part, red);
-    if (tid == 0) {
-        const c128 alpha = xs[0];
-        c128 tau = cmake(0.0, 0.0), s = cmake(0.0, 0.0);
-        double beta = alpha.x;
-        if (xnorm2 > 0.0 || alpha.y != 0.0) {
-            beta = -copysign(sqrt(alpha.x * alpha.x + alpha.y * alpha.y + xnorm2), alpha.x);
-            tau = cmake((beta - alpha.x) / beta, -alpha.y / beta);
-            const double dr = alpha.x - beta, di = alpha.y;
-            const double den = dr * dr + di * di;
-            s = cmake(dr / den, -di / den);
-        }
-        scal[0] = tau; scal[1] = s; scal[2] = cmake(beta, 0.0);
+// One chase step (sweep j, step k) by the compute group.  FULL: len = len2 = 64 (no edge predicates).
+// Returns false when the sweep ended with this step (no S block below).
+template <bool FULL>
+__device__ __forceinline__ bool bc_step(BcSmem& sm, const BcStepCtx& t, int r0, int len_, int len2_, int k, c128& tau) {
+    const int len = FULL ? BC_B : len_, len2 = FULL ? BC_B : len2_;
+    const int r = t.r, q = t.q, rl = t.rl;
+    c128* const band = t.band;
+    const int64_t ldab = t.ldab;
+    // ---- D_k: lower triangle, global -> shared (asynchronous, through L2)
+#pragma unroll
+    for (int it = 0; it < BC_B * BC_B / BC_NT; ++it) {
+        const int idx = t.tid + it * BC_NT;
+        const int rr = idx & (BC_B - 1), cc = idx >> 6;
+        if (rr >= cc && (FULL || rr < len))
+            cp_async16(&sm.D[rr + cc * BC_LD], band + (rr - cc) + (int64_t)(r0 + cc) * ldab, 16);
     }
-    __syncthreads();
-    const c128 tau = scal[0], s = scal[1];
-    *beta_out = scal[2].x;
-    c128 x = cmake(0.0, 0.0);
-    if (tid < len) x = xs[tid];
-    __syncthreads();       // xs may alias vs
-    if (tid < len) vs[tid] = (tid == 0) ? cmake(1.0, 0.0) : cmul(s, x);
-    __syncthreads();
-    return tau;
-}
-
-__device__ __forceinline__ void bc_wait(const int* progress, int sweep, int need) {
-    if (sweep >= 0) {
-        if (threadIdx.x == 0) {
-            while (*(volatile const int*)(progress + sweep) < need) {}
-            __threadfence();
+    cp_async_commit();
+    // ---- S_{k+1}: rows r0+b+r, cols r0+c -> registers
+    c128 sreg[BC_NC];
+    {
+        const c128* sp = band + (BC_B + r - q) + (int64_t)(r0 + q) * ldab;    // element (r, c = q); next c: + 4 (ldab - 1)
+#pragma unroll
+        for (int i = 0; i < BC_NC; ++i) {
+            sreg[i] = cmake(0.0, 0.0);
+            if (FULL || (r < len2 && q + 4 * i < len)) sreg[i] = __ldcg(sp + (int64_t)i * 4 * (ldab - 1));
         }
     }
-    __syncthreads();
+    cp_async_wait<0>();
+    bc_sync_compute();                                   // D landed; vs of this step visible
+    c128 vc[BC_NC];
+#pragma unroll
+    for (int i = 0; i < BC_NC; ++i) vc[i] = sm.vs[q + 4 * i];
+    const c128 vr = sm.vs[r];
+    // ---- w = D v (Hermitian D from its lower triangle), four independent accumulators
+    c128 wr;
+    {
+        c128 acc[4];
+#pragma unroll
+        for (int u = 0; u < 4; ++u) acc[u] = cmake(0.0, 0.0);
+#pragma unroll
+        for (int i = 0; i < BC_NC; ++i) {
+            const int c = q + 4 * i;
+            c128 e = cmake(0.0, 0.0);
+            if (FULL || (r < len && c < len)) {
+                e = sm.D[c <= r ? r + c * BC_LD : c + r * BC_LD];
+                if (c >= r) e.y = (c == r) ? 0.0 : -e.y;
+            }
+            cfma(acc[i & 3], e, vc[i]);
+        }
+        wr = cadd(cadd(acc[0], acc[1]), cadd(acc[2], acc[3]));
+    }
+    wr = cadd(wr, bc_shfl_xor(wr, 8));
+    wr = cadd(wr, bc_shfl_xor(wr, 16));
+    {
+        double pa = (q == 0) ? vr.x * wr.x + vr.y * wr.y : 0.0;   // Re(conj(v_r) w_r)
+        pa = bc_warp_sum(pa);
+        if (t.lane == 0) sm.red[t.warp] = pa;
+        if (q == 0) sm.ws[r] = wr;
+    }
+    bc_sync_compute();
+    {
+        double vhw = 0.0;
+#pragma unroll
+        for (int w = 0; w < BC_NW; ++w) vhw += sm.red[w];
+        // y = tau w - f v, f = 1/2 |tau|^2 (v^H w);  D -= v y^H + y v^H = (conj(tau) v_r) conj(w_c) + (tau w_r - 2 f v_r) conj(v_c)
+        const double f2 = (tau.x * tau.x + tau.y * tau.y) * vhw;
+        const c128 pr = cmulc(tau, vr);                    // conj(tau) v_r
+        const c128 twr = cmul(tau, wr);
+        const c128 qr = cmake(twr.x - f2 * vr.x, twr.y - f2 * vr.y);
+        if (FULL || r < len) {
+            c128* dp = band + (r - q) + (int64_t)(r0 + q) * ldab;
+#pragma unroll
+            for (int i = 0; i < BC_NC; ++i) {
+                const int c = q + 4 * i;
+                if (c <= r) {
+                    const c128 wc = sm.ws[c];
+                    c128 e = sm.D[r + c * BC_LD];
+                    e.x -= pr.x * wc.x + pr.y * wc.y + qr.x * vc[i].x + qr.y * vc[i].y;
+                    e.y -= pr.y * wc.x - pr.x * wc.y + qr.y * vc[i].x - qr.x * vc[i].y;
+                    if (c == r) e.y = 0.0;
+                    dp[(int64_t)i * 4 * (ldab - 1)] = e;
+                }
+            }
+        }
+    }
+    if (!FULL && len2 <= 0) return false;
+    // ---- S <- S (I - tau v v^H):  u = S v,  S -= (tau u) v^H   (all in registers)
+    {
+        c128 acc[4];
+#pragma unroll
+        for (int u = 0; u < 4; ++u) acc[u] = cmake(0.0, 0.0);
+#pragma unroll
+        for (int i = 0; i < BC_NC; ++i) cfma(acc[i & 3], sreg[i], vc[i]);
+        c128 ur = cadd(cadd(acc[0], acc[1]), cadd(acc[2], acc[3]));
+        ur = cadd(ur, bc_shfl_xor(ur, 8));
+        ur = cadd(ur, bc_shfl_xor(ur, 16));
+        const c128 tu = cmul(tau, ur);
+#pragma unroll
+        for (int i = 0; i < BC_NC; ++i) {
+            sreg[i].x -= tu.x * vc[i].x + tu.y * vc[i].y;
+            sreg[i].y -= tu.y * vc[i].x - tu.x * vc[i].y;
+        }
+    }
+    // ---- next reflector from the first column of S (held by the q = 0 lanes in sreg[0])
+    c128 taun;
+    double betan;
+    c128 vnr;
+    {
+        const c128 x = cmake(__shfl_sync(0xffffffffu, sreg[0].x, rl), __shfl_sync(0xffffffffu, sreg[0].y, rl));
+        vnr = bc_make_reflector(x, t, len2, sm.red2, &sm.xs[0], taun, betan);
+    }
+    // ---- z_c = vn^H S[:, c]: per-thread products, reduce-scatter over the 8 row lanes, then across warps
+    {
+        c128 zp[BC_NC];
+#pragma unroll
+        for (int i = 0; i < BC_NC; ++i) zp[i] = cmulc(vnr, sreg[i]);
+#pragma unroll
+        for (int st = 0; st < 3; ++st) {
+            const int half = BC_NC >> (st + 1);
+            const bool up = (rl >> st) & 1;
+#pragma unroll
+            for (int i = 0; i < half; ++i) {
+                const c128 send = up ? zp[i] : zp[i + half];
+                const c128 keep = up ? zp[i + half] : zp[i];
+                zp[i] = cadd(keep, bc_shfl_xor(send, 1 << st));
+            }
+        }
+        // zp[i'] (i' = 0, 1) is the sum over the warp's rows of column index i = i' + 2 b2 + 4 b1 + 8 b0
+        const int ibase = ((rl >> 2) & 1) * 2 + ((rl >> 1) & 1) * 4 + (rl & 1) * 8;
+        sm.zpart[t.warp * BC_B + q + 4 * (ibase + 0)] = zp[0];
+        sm.zpart[t.warp * BC_B + q + 4 * (ibase + 1)] = zp[1];
+    }
+    bc_sync_compute();
+    if (t.tid < BC_B) {
+        c128 z0 = cadd(sm.zpart[0 * BC_B + t.tid], sm.zpart[1 * BC_B + t.tid]);
+        c128 z1 = cadd(sm.zpart[2 * BC_B + t.tid], sm.zpart[3 * BC_B + t.tid]);
+        c128 z2 = cadd(sm.zpart[4 * BC_B + t.tid], sm.zpart[5 * BC_B + t.tid]);
+        c128 z3 = cadd(sm.zpart[6 * BC_B + t.tid], sm.zpart[7 * BC_B + t.tid]);
+        sm.zs[t.tid] = cmulc(taun, cadd(cadd(z0, z1), cadd(z2, z3)));        // conj(tau') z_c
+    }
+    bc_sync_compute();
+    // ---- S[:, c] -= vn (conj(tau') z_c) for c >= 1; S[:, 0] = beta' e_1; store S and the reflector
+    {
+        c128* sp = band + (BC_B + r - q) + (int64_t)(r0 + q) * ldab;
+#pragma unroll
+        for (int i = 0; i < BC_NC; ++i) {
+            const int c = q + 4 * i;
+            c128 e = sreg[i];
+            if (c == 0) e = (r == 0) ? cmake(betan, 0.0) : cmake(0.0, 0.0);
+            else {
+                const c128 zc = sm.zs[c];
+                e.x -= vnr.x * zc.x - vnr.y * zc.y;
+                e.y -= vnr.x * zc.y + vnr.y * zc.x;
+            }
+            if (FULL || (r < len2 && c < len)) sp[(int64_t)i * 4 * (ldab - 1)] = e;
+        }
+    }
+    if (q == 0) {
+        if (FULL || r < len2) t.Vj[r0 + BC_B + r] = vnr;
+        sm.vs[r] = vnr;
+    }
+    if (t.tid == 0) t.tau2j[k + 1] = taun;
+    tau = taun;
+    return true;
 }
 
-__global__ void __launch_bounds__(BC_NT, 1) bulge_chase_kernel(const BcArgs a) {
+__global__ void __launch_bounds__(BC_NT + 32, 1) bulge_chase_kernel(const BcArgs a) {
     extern __shared__ __align__(16) unsigned char bc_raw[];
-    c128* D = reinterpret_cast<c128*>(bc_raw);      // [BC_B][BC_LD]
-    c128* S = D + BC_B * BC_LD;                     // [BC_B][BC_LD]
-    c128* v = S + BC_B * BC_LD;                     // [BC_B]
-    c128* vn = v + BC_B;                            // [BC_B]
-    c128* w = vn + BC_B;                            // [BC_B]
-    c128* y = w + BC_B;                             // [BC_B]
-    c128* wpart = y + BC_B;                         // [4][BC_B]
-    c128* scal = wpart + 4 * BC_B;                  // [4]
-    double* red = reinterpret_cast<double*>(scal + 4);   // [8]
+    BcSmem& sm = *reinterpret_cast<BcSmem*>(bc_raw);
 
-    const int tid = threadIdx.x;
-    const int r = tid & 63, q = tid >> 6;           // row / quarter
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int N = a.N;
-    const int64_t ldab = a.ldab;
+
+    if (warp == BC_NW) {
+        // ================= publisher warp: one release per completed step, INT_MAX per completed sweep
+        int hb = 0;
+        for (int j = blockIdx.x; j <= N - 2; j += gridDim.x) {
+            for (int k = 0;; ++k) {
+                const bool more = N - (j + 1 + k * BC_B + BC_B) > 0;
+                bc_handoff_wait(hb);
+                hb ^= 1;
+                if (lane == 0) bc_st_release(a.progress + j, more ? k + 1 : INT_MAX);
+                if (!more) break;
+            }
+        }
+        return;
+    }
+
+    BcStepCtx t;
+    t.band = a.band; t.ldab = a.ldab;
+    t.tid = tid; t.lane = lane; t.warp = warp;
+    t.rl = lane & 7; t.q = lane >> 3; t.r = warp * 8 + t.rl;
+    const int r = t.r, q = t.q;
+    int hb = 0;
 
     for (int j = blockIdx.x; j <= N - 2; j += gridDim.x) {
         const int64_t voff = (int64_t)j * (N - 1) - (int64_t)j * (j - 1) / 2;   // packed column j
-        c128* Vj = a.V2 + voff - j - 1;              // Vj[row] for row in j+1..N-1
-        bc_wait(a.progress, j - 1, 2);
-        int len = min(BC_B, N - 1 - j);
-        // ---- step 0: reflector from column j
-        c128* colj = a.band + (int64_t)j * ldab;
-        if (tid < len) v[tid] = __ldcg(colj + 1 + tid);
-        __syncthreads();
-        double beta;
-        c128 tau = bc_make_reflector(v, v, len, red, scal, &beta);
-        if (tid < len) {
-            colj[1 + tid] = (tid == 0) ? cmake(beta, 0.0) : cmake(0.0, 0.0);
-            Vj[j + 1 + tid] = v[tid];
-            if (tid == 0) a.tau2[(int64_t)j * a.kmax] = tau;
+        t.Vj = a.V2 + voff - j - 1;                  // Vj[row] for row in j+1..N-1
+        t.tau2j = a.tau2 + (int64_t)j * a.kmax;
+        if (tid == 0) bc_poll(a.progress, j - 1, 2);
+        bc_sync_compute();
+        // ---- reflector (j, 0) from column j of the band
+        c128 tau;
+        {
+            const int len = min(BC_B, N - 1 - j);
+            c128* colj = a.band + (int64_t)j * a.ldab;
+            c128 x = cmake(0.0, 0.0);
+            if (r < len) x = __ldcg(colj + 1 + r);
+            double beta;
+            const c128 vr = bc_make_reflector(x, t, len, sm.red2, &sm.xs[0], tau, beta);
+            if (q == 0) {
+                if (r < len) {
+                    colj[1 + r] = (r == 0) ? cmake(beta, 0.0) : cmake(0.0, 0.0);
+                    t.Vj[j + 1 + r] = vr;
+                }
+                sm.vs[r] = vr;
+            }
+            if (tid == 0) t.tau2j[0] = tau;
         }
         for (int k = 0;; ++k) {
             const int r0 = j + 1 + k * BC_B;
-            len = min(BC_B, N - r0);
-            if (k > 0) bc_wait(a.progress, j - 1, k + 2);
-            // ---- load D_k (lower from band, mirrored)
-            for (int cc = q; cc < len; cc += 4) {
-                if (r < len && r >= cc) {
-                    c128 e = __ldcg(a.band + (r - cc) + (int64_t)(r0 + cc) * ldab);
-                    if (r == cc) e.y = 0.0;
-                    D[r + cc * BC_LD] = e;
-                    if (r != cc) D[cc + r * BC_LD] = cconj(e);
-                }
-            }
-            __syncthreads();
-            // ---- w = D v
-            {
-                c128 acc = cmake(0.0, 0.0);
-                if (r < len)
-                    for (int cc = q * 16; cc < min(len, q * 16 + 16); ++cc) cfma(acc, D[r + cc * BC_LD], v[cc]);
-                wpart[q * BC_B + r] = acc;
-            }
-            __syncthreads();
-            if (tid < BC_B) {
-                c128 s = cmake(0.0, 0.0);
-                if (tid < len) s = cadd(cadd(wpart[tid], wpart[BC_B + tid]), cadd(wpart[2 * BC_B + tid], wpart[3 * BC_B + tid]));
-                w[tid] = s;
-            }
-            __syncthreads();
-            // alpha = v^H w (real)
-            double pa = 0.0;
-            if (tid < len) pa = v[tid].x * w[tid].x + v[tid].y * w[tid].y;
-            const double vhw = bc_block_sum(pa, red);
-            // y = tau w - 1/2 |tau|^2 alpha v
-            if (tid < len) {
-                const double f = 0.5 * (tau.x * tau.x + tau.y * tau.y) * vhw;
-                const c128 tw = cmul(tau, w[tid]);
-                y[tid] = cmake(tw.x - f * v[tid].x, tw.y - f * v[tid].y);
-            }
-            __syncthreads();
-            // D <- D - v y^H - y v^H ; store lower
-            if (r < len) {
-                const c128 vr = v[r], yr = y[r];
-                for (int cc = q; cc < len; cc += 4) {
-                    if (r >= cc) {
-                        c128 e = D[r + cc * BC_LD];
-                        const c128 yc = y[cc], vc = v[cc];
-                        // v_r conj(y_c) + y_r conj(v_c)
-                        e.x -= vr.x * yc.x + vr.y * yc.y + yr.x * vc.x + yr.y * vc.y;
-                        e.y -= vr.y * yc.x - vr.x * yc.y + yr.y * vc.x - yr.x * vc.y;
-                        if (r == cc) e.y = 0.0;
-                        a.band[(r - cc) + (int64_t)(r0 + cc) * ldab] = e;
-                    }
-                }
-            }
+            const int len = min(BC_B, N - r0);
             const int len2 = min(BC_B, N - (r0 + BC_B));
-            if (len2 <= 0) break;
-            // ---- load S_{k+1}: rows r0+b+ii (ii < len2), cols r0+cc (cc < len)
-            for (int cc = q; cc < len; cc += 4)
-                if (r < len2) S[r + cc * BC_LD] = __ldcg(a.band + (BC_B + r - cc) + (int64_t)(r0 + cc) * ldab);
-            __syncthreads();
-            // u = S v  (len2)
-            {
-                c128 acc = cmake(0.0, 0.0);
-                if (r < len2)
-                    for (int cc = q * 16; cc < min(len, q * 16 + 16); ++cc) cfma(acc, S[r + cc * BC_LD], v[cc]);
-                wpart[q * BC_B + r] = acc;
-            }
-            __syncthreads();
-            if (tid < BC_B) {
-                c128 s = cmake(0.0, 0.0);
-                if (tid < len2) s = cadd(cadd(wpart[tid], wpart[BC_B + tid]), cadd(wpart[2 * BC_B + tid], wpart[3 * BC_B + tid]));
-                w[tid] = cmul(tau, s);      // tau * u
-            }
-            __syncthreads();
-            // S <- S - (tau u) v^H
-            if (r < len2) {
-                const c128 ur = w[r];
-                for (int cc = q; cc < len; cc += 4) {
-                    c128 e = S[r + cc * BC_LD];
-                    const c128 vc = v[cc];
-                    e.x -= ur.x * vc.x + ur.y * vc.y;
-                    e.y -= ur.y * vc.x - ur.x * vc.y;
-                    S[r + cc * BC_LD] = e;
-                }
-            }
-            __syncthreads();
-            // ---- next reflector from S[:,0]
-            double betan;
-            if (tid < len2) vn[tid] = S[tid];
-            __syncthreads();
-            const c128 taun = bc_make_reflector(vn, vn, len2, red, scal, &betan);
-            if (tid < len2) S[tid] = (tid == 0) ? cmake(betan, 0.0) : cmake(0.0, 0.0);
-            // z_c = vn^H S[:,c], c = 1..len-1 : thread (c = r, rows quarter q)
-            {
-                c128 acc = cmake(0.0, 0.0);
-                if (r >= 1 && r < len)
-                    for (int ii = q * 16; ii < min(len2, q * 16 + 16); ++ii) cfmac(acc, vn[ii], S[ii + r * BC_LD]);
-                wpart[q * BC_B + r] = acc;
-            }
-            __syncthreads();
-            if (tid < BC_B) {
-                c128 s = cmake(0.0, 0.0);
-                if (tid >= 1 && tid < len) s = cadd(cadd(wpart[tid], wpart[BC_B + tid]), cadd(wpart[2 * BC_B + tid], wpart[3 * BC_B + tid]));
-                w[tid] = cmulc(taun, s);    // conj(tau') z_c
-            }
-            __syncthreads();
-            // S[:,c] -= vn (conj(tau') z_c), c >= 1 ; store S
-            if (r < len2) {
-                const c128 vr = vn[r];
-                for (int cc = q; cc < len; cc += 4) {
-                    c128 e = S[r + cc * BC_LD];
-                    if (cc >= 1) {
-                        const c128 t = cmul(vr, w[cc]);
-                        e.x -= t.x; e.y -= t.y;
-                    }
-                    a.band[(BC_B + r - cc) + (int64_t)(r0 + cc) * ldab] = e;
-                }
-            }
-            if (tid < len2) Vj[r0 + BC_B + tid] = vn[tid];
-            if (tid == 0) a.tau2[(int64_t)j * a.kmax + k + 1] = taun;
-            __syncthreads();
-            if (tid == 0) {
-                __threadfence();
-                *(volatile int*)(a.progress + j) = k + 1;
-            }
-            // v <- vn
-            if (tid < BC_B) v[tid] = (tid < len2) ? vn[tid] : cmake(0.0, 0.0);
-            tau = taun;
-            __syncthreads();
+            const bool more = (len == BC_B && len2 == BC_B) ? bc_step<true>(sm, t, r0, len, len2, k, tau)
+                                                            : bc_step<false>(sm, t, r0, len, len2, k, tau);
+            // all band / reflector stores of this step are issued: hand the release to the publisher warp
+            bc_handoff_arrive(hb);
+            hb ^= 1;
+            if (!more) break;
+            if (tid == 0) bc_poll(a.progress, j - 1, k + 3);
+            bc_sync_compute();
         }
-        __syncthreads();
-        if (tid == 0) {
-            __threadfence();
-            *(volatile int*)(a.progress + j) = INT_MAX;
-        }
-        __syncthreads();
     }
 }
 
@@ -285,22 +394,23 @@ int phase_band_to_tridiag(eigh_handle_s* h, c128* band, int64_t ldab, double* d,
     double* sgn = ws_ptr<double>(h, pl.sgn);
     EIGH_CUDA_OK(cudaMemsetAsync(progress, 0, (size_t)(N + 8) * sizeof(int), s));
     if (N >= 2) {
-        const size_t smem = (size_t)(2 * BC_B * BC_LD + 4 * BC_B + 4 * BC_B + 4) * sizeof(c128) + 8 * sizeof(double);
+        const size_t smem = sizeof(BcSmem);
         static bool attr = false;
         if (!attr) {
             EIGH_CUDA_OK(cudaFuncSetAttribute(bulge_chase_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
             attr = true;
         }
         int occ = 0;
-        EIGH_CUDA_OK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, bulge_chase_kernel, BC_NT, smem));
+        EIGH_CUDA_OK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, bulge_chase_kernel, BC_NT + 32, smem));
         if (occ < 1) return set_err(h, EIGH_ERR_CUDA, "bulge_chase_kernel cannot be resident");
         int G = h->num_sms * occ;
+        if (h->bc_grid > 0 && h->bc_grid < G) G = h->bc_grid;
         if (G > N - 1) G = N - 1;
         BcArgs a;
         a.band = band; a.ldab = ldab; a.N = N; a.V2 = ws_ptr<c128>(h, pl.V2); a.progress = progress;
         a.tau2 = ws_ptr<c128>(h, pl.tau2); a.kmax = (int)bc_kmax(h);
         void* kargs[] = {(void*)&a};
-        EIGH_CUDA_OK(cudaLaunchCooperativeKernel((void*)bulge_chase_kernel, dim3(G), dim3(BC_NT), kargs, smem, s));
+        EIGH_CUDA_OK(cudaLaunchCooperativeKernel((void*)bulge_chase_kernel, dim3(G), dim3(BC_NT + 32), kargs, smem, s));
         ++h->launches;
     }
     extract_tridiag_kernel<<<(unsigned)ceil_div(N, 256), 256, 0, s>>>(band, ldab, N, d, e, sgn);

@@ -41,6 +41,7 @@ struct eigh_handle_s {
     int g;          // WY group size for S4a
     int leaf;       // D&C leaf size
     int p4b_merge;  // panels per WY block in S4b
+    int bc_grid;    // S2: CTAs of the bulge-chasing kernel (0 = all that are co-resident)
     int64_t ldab;   // band storage leading dimension
     void* ws;
     size_t ws_bytes;
