@@ -172,6 +172,7 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--wy-group", type=int, default=0)
+    ap.add_argument("--opt", action="append", default=[], help="solver option key=value (eigh_set_option), repeatable")
     args = ap.parse_args()
     if args.warmup < 3 and args.impl != "reference":
         args.warmup = max(args.warmup, 1)
@@ -201,6 +202,9 @@ def main():
     opts = {}
     if args.wy_group:
         opts["wy_group"] = args.wy_group
+    for kv in args.opt:
+        key, val = kv.split("=")
+        opts[key] = int(val)
     solver = binding.Eigh(N, nev, device=dev, **opts)
     b = 64
     mat_bytes = N * N * 16

@@ -42,7 +42,8 @@ int eigh_create(eigh_handle_t* h, int64_t N, int64_t nev);
 
 /* Tuning knobs; must be called before eigh_workspace_size.  Keys: "band_width" (64 or 128),
  * "wy_group" (reflectors per compact-WY block of S4a: 8, 16 or 32), "dc_leaf" (8..32), "p4b_merge" (1..4 panels of S1 merged into one compact-WY block of S4b; default 4),
- * "bc_grid" (thread blocks of the S2 bulge-chasing kernel; 0 = every co-resident block, the default).
+ * "bt_chain" (S4a: consecutive passes of one column slab scheduled back to back so that followers read from L2;
+ * 0 = automatic), "bc_grid" (thread blocks of the S2 bulge-chasing kernel; 0 = every co-resident block, the default).
  * Returns -2 for an unknown key, -3 for a bad value. */
 int eigh_set_option(eigh_handle_t h, const char* key, int64_t value);
 

@@ -48,7 +48,8 @@ void plan_workspace(eigh_handle_s* h) {
     p.X = bump(off, (size_t)N * b * sizeof(c128));
     p.small = bump(off, (size_t)4 * b * b * sizeof(c128));
     p.panel_sync = bump(off, (size_t)(256 + 2 * 160 * (2 * b + 8) * sizeof(c128)));
-    p.V2 = bump(off, (size_t)(N * (N - 1) / 2 + 2 * b) * sizeof(c128));
+    p.V2 = bump(off, (size_t)(v2_total_stages(N) * 32 * 64 + 64) * sizeof(c128));
+    p.pass_off = bump(off, (size_t)(v2_npass(N) + 8) * sizeof(int64_t));
     p.tau2 = bump(off, (size_t)N * bc_kmax(h) * sizeof(c128));
     p.bc_progress = bump(off, (size_t)(N + 8) * sizeof(int));
     p.d = bump(off, (size_t)N * sizeof(double));
@@ -116,6 +117,9 @@ int eigh_set_option(eigh_handle_t h, const char* key, int64_t value) {
     } else if (!strcmp(key, "p4b_merge")) {
         if (value < 1 || value > 4) return set_err(h, -3, "p4b_merge must be in [1, 4]");
         h->p4b_merge = (int)value;
+    } else if (!strcmp(key, "bt_chain")) {
+        if (value < 0 || value > 16) return set_err(h, -3, "bt_chain must be in [0, 16]");
+        h->bt_chain = (int)value;
     } else if (!strcmp(key, "bc_grid")) {
         if (value < 0 || value > 4096) return set_err(h, -3, "bc_grid must be in [0, 4096]");
         h->bc_grid = (int)value;

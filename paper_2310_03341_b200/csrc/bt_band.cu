@@ -21,14 +21,24 @@
 //  * Only the 8x8 blocks of V inside the parallelogram are multiplied (9 row blocks per column
 //    block instead of 12): executed/credited flops = 9/8 (+ the small T product).
 //  * V (packed, straight from bulge chasing) and -T (prepared per (pass, k)) reach shared memory by
-//    1-D bulk async copies (cp.async.bulk, SASS UBLKCP) issued by a producer warp into a 3-stage
-//    ring guarded by full/empty mbarriers; the 8 consumer warps never meet at a CTA barrier.
+//    1-D bulk async copies (cp.async.bulk, SASS UBLKCP) into a 3-stage ring guarded by full/empty
+//    mbarriers.  There is no producer warp (a ninth warp would cap every thread at 168 registers:
+//    three warps on one SM sub-partition): lane 0 of warp 0 issues the copies of stage it+2 at the
+//    top of step it.  The 8 warps never meet at a CTA barrier.
 //    Shared-memory leading dimensions are odd (97, 33), which makes both fragment access patterns
 //    (row-fastest for V^H Z, column-fastest for V Y) conflict-free for 128-bit loads.
 //  * Z rows enter and leave the register window straight from/to global memory: the window slides
-//    down by 64 rows per step, so every row of Z is read once and written once per pass.
-//  * Units are handed out by an atomic counter in (pass descending, slab) order; (pass, slab)
-//    waits for (pass+1, slab) through a per-slab completion counter in global memory.
+//    down by 64 rows per step, so every row of Z is read once and written once per pass.  The 64
+//    rows of the next step are fetched into a second register set BEFORE the products of the
+//    current step, so their latency is hidden behind ~30k cycles of DMMA work.
+//  * Units are handed out by an atomic counter.  Dependencies are per (pass, slab, warp) -- a warp
+//    owns its 8 columns for the whole unit, so it only ever depends on the same warp index of the
+//    unit (pass+1, slab): step k of pass p-1 reads rows that pass p finalises in its step k.  Every
+//    warp publishes "steps completed" with a release store (delayed by one step so that the fence
+//    finds the stores already drained) and polls its predecessor with ld.acquire.
+//  * Unit order: groups of `chain` consecutive passes; inside a group slab-major, so that the
+//    chain members of one slab run concurrently on neighbouring CTAs, a few steps apart, and the
+//    followers read from L2 what the leader has just written (HBM traffic / chain).
 #include "eigh_internal.h"
 
 namespace eigh {
@@ -37,20 +47,27 @@ constexpr int BT_B = 64;            // band width (reflector length)
 constexpr int BT_P = 32;            // sweeps per pass
 constexpr int BT_WR = BT_B + BT_P;  // window rows (96)
 constexpr int BT_NBLK = BT_WR / 8;  // 12 row blocks
-constexpr int BT_LDV = BT_WR + 1;   // 97, odd
+constexpr int BT_LDV = BT_B - 1;    // 63: element (window row R, reflector c) of a stage at 63 c + R (valid for 0 <= R - c < 64),
+                                    // i.e. the stage is the plain [32][64] tile of the reflector storage; odd => conflict-free
 constexpr int BT_LDT = BT_P + 1;    // 33, odd
-constexpr int BT_VS = BT_LDV * BT_P;        // c128 per V stage
+constexpr int BT_VS = BT_B * BT_P;          // c128 per V stage (32 KB)
 constexpr int BT_TS = BT_LDT * BT_P;        // c128 per T stage
-constexpr int BT_STAGES = 3;
-constexpr int BT_CWARPS = 8;                // consumer warps
-constexpr int BT_NT = 32 * (BT_CWARPS + 1); // + producer warp
+constexpr int BT_LDZ = BT_B + 1;            // 65, odd: per-warp staging of the 64 incoming rows of 8 columns
+constexpr int BT_ZS = 8 * BT_LDZ;           // c128 per warp
+// compact -T of one (pass, k) step for WY blocks of GS reflectors: 32/GS blocks [GS x GS], ld GS+1
+__host__ __device__ constexpr int bt_tsz(int gs) { return BT_P * (gs + 1); }
+__host__ __device__ constexpr int bt_stages(int gs) { return gs == 32 ? 3 : 4; }
+constexpr int BT_CWARPS = 8;                // warps per CTA (all of them consumers)
+constexpr int BT_NT = 32 * BT_CWARPS;
 constexpr int BT_SLAB = 8 * BT_CWARPS;      // 64 columns per unit
 
-struct BtHeader { int j0, k, slab, flags; };   // flags: 1 first step of unit, 2 last step, 4 terminate
-constexpr size_t BT_SMEM = (size_t)BT_STAGES * (BT_VS + BT_TS) * sizeof(c128) + BT_STAGES * sizeof(BtHeader) +
-                           2 * BT_STAGES * sizeof(uint64_t) + 64;
+struct BtHeader { int j0, k, slab, flags, pass, nk_pred, pad0, pad1; };   // flags: 1 first step of unit, 2 last step, 4 terminate
+__host__ __device__ constexpr size_t bt_smem(int gs) {
+    return (size_t)bt_stages(gs) * (BT_VS + bt_tsz(gs)) * sizeof(c128) + (size_t)BT_CWARPS * BT_ZS * sizeof(c128) +
+           bt_stages(gs) * sizeof(BtHeader) + (2 * bt_stages(gs) + BT_CWARPS) * sizeof(uint64_t) + 64;
+}
 
-static inline int64_t bt_npass(int64_t N) { return N >= 2 ? ceil_div(N - 1, BT_P) : 0; }
+static inline int64_t bt_npass(int64_t N) { return v2_npass(N); }
 
 size_t bt_tneg_bytes(int64_t N) {
     // stages = sum over passes of ceil((N-1-j0)/64)  <=  npass * kmax
@@ -59,9 +76,10 @@ size_t bt_tneg_bytes(int64_t N) {
     return (size_t)st * BT_TS * sizeof(c128) + 256;
 }
 size_t bt_scratch_bytes(const eigh_handle_s* h) {
-    // pass offsets + unit counter + per-slab completion counters + S4b's Y
+    // S4b's Y + pass offsets + unit counter + per (pass, slab, warp) progress counters
     const size_t y = (size_t)h->b * h->nev * sizeof(c128);
-    return y + (size_t)(bt_npass(h->N) + 8) * sizeof(int64_t) + (size_t)(ceil_div(h->nev, BT_SLAB) + 64) * sizeof(int) + 8192;
+    const size_t prog = (size_t)bt_npass(h->N) * ceil_div(h->nev, BT_SLAB) * BT_CWARPS * sizeof(int);
+    return y + (size_t)(bt_npass(h->N) + 8) * sizeof(int64_t) + prog + 8192;
 }
 
 // ------------------------------------------------------------------ small kernels
@@ -110,8 +128,7 @@ __global__ void __launch_bounds__(128) bt_tprep_kernel(const c128* __restrict__ 
         const int r0 = j + 1 + k * BT_B;
         const int len = min(BT_B, N - r0);
         if (j <= N - 2 && i < len) {
-            const int64_t voff = (int64_t)j * (N - 1) - (int64_t)j * (j - 1) / 2;
-            Vs[(t + i) + t * BT_WR] = V2[voff + (int64_t)k * BT_B + i];
+            Vs[(t + i) + t * BT_WR] = V2[((pass_off[pass] + k) * BT_P + t) * BT_B + i];
         }
     }
     if (tid < BT_P) {
@@ -143,10 +160,13 @@ __global__ void __launch_bounds__(128) bt_tprep_kernel(const c128* __restrict__ 
     }
     __syncthreads();
     c128* out = Tneg + (size_t)(pass_off[pass] + k) * BT_TS;
-    for (int idx = tid; idx < BT_TS; idx += 128) {
-        const int o = idx % BT_LDT, in = idx / BT_LDT;
+    // compact layout: block s = reflectors [s gs, (s+1) gs); element (o, in) of block s at s gs (gs+1) + o + in (gs+1)
+    const int ldc = gs + 1;
+    for (int idx = tid; idx < BT_P * ldc; idx += 128) {
+        const int blk = idx / (gs * ldc), rem = idx % (gs * ldc);
+        const int o = rem % ldc, in = rem / ldc;
         c128 v = cmake(0.0, 0.0);
-        if (o < BT_P) { const c128 t = Ts[o + in * (BT_P + 1)]; v = cmake(-t.x, -t.y); }
+        if (o < gs) { const c128 t = Ts[(blk * gs + o) + (blk * gs + in) * (BT_P + 1)]; v = cmake(-t.x, -t.y); }
         out[idx] = v;
     }
 }
@@ -181,6 +201,15 @@ __device__ __forceinline__ void bulk_g2s(void* dst, const void* src, uint32_t by
                  "l"(src), "r"(bytes), "r"(smem_u32(b))
                  : "memory");
 }
+__device__ __forceinline__ void bulk_s2g(void* gdst, const void* ssrc, uint32_t bytes) {
+    asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;" ::"l"(gdst), "r"(smem_u32(ssrc)), "r"(bytes)
+                 : "memory");
+}
+__device__ __forceinline__ void bulk_commit() { asm volatile("cp.async.bulk.commit_group;" ::: "memory"); }
+template <int N>
+__device__ __forceinline__ void bulk_wait_read() { asm volatile("cp.async.bulk.wait_group.read %0;" ::"n"(N) : "memory"); }
+template <int N>
+__device__ __forceinline__ void bulk_wait() { asm volatile("cp.async.bulk.wait_group %0;" ::"n"(N) : "memory"); }
 // pure (non-volatile) DMMA so that the compiler may schedule it freely
 __device__ __forceinline__ void dmma_p(double (&c)[2], double a, double b) {
     asm("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};\n"
@@ -194,21 +223,32 @@ struct BtSweepArgs {
     const c128* V2;
     const c128* Tneg;
     const int64_t* pass_off;
-    int npass, nslabs;
+    int npass, nslabs, chain;
     unsigned long long* unit_counter;   // zero on entry
-    int* slab_done;                     // [nslabs], zero on entry; += 8 per finished (pass, slab)
+    int* prog;                          // [npass][nslabs][8], zero on entry: steps completed by (pass, slab, warp)
 };
+
+__device__ __forceinline__ int bt_ld_acquire(const int* p) {
+    int v;
+    asm volatile("ld.acquire.gpu.global.s32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
+    return v;
+}
+__device__ __forceinline__ void bt_st_release(int* p, int v) {
+    asm volatile("st.release.gpu.global.s32 [%0], %1;" ::"l"(p), "r"(v) : "memory");
+}
 
 // ------------------------------------------------------------------ the sweeper
 // One (pass, k) step on the register window.  GS = reflectors per compact-WY block (8, 16 or 32).
-template <int GS>
+template <int GS, int S_HI, int S_LO>
 __device__ __forceinline__ void bt_apply_step(const c128* __restrict__ Vs, const c128* __restrict__ Ts,
                                               double (&zr)[BT_NBLK][2], double (&zi)[BT_NBLK][2], int g, int t,
                                               bool tail, int nrows) {
     constexpr int NB = GS / 8;          // column blocks per WY block
     constexpr int NSUB = BT_P / GS;
 #pragma unroll
-    for (int s = NSUB - 1; s >= 0; --s) {
+    static_assert(S_HI < NSUB && S_LO >= 0, "sub-block range");
+#pragma unroll
+    for (int s = S_HI; s >= S_LO; --s) {
         const int cb0 = s * NB;
         // ---- Y1 = V^H Z   (m = column of Z, n = reflector, k = row)
         double y1r[NB][2][2], y1i[NB][2][2];   // [col block][k-step parity h][frag]
@@ -225,7 +265,10 @@ __device__ __forceinline__ void bt_apply_step(const c128* __restrict__ Vs, const
                 for (int c = 0; c < NB; ++c) {
                     const int cb = cb0 + c;
                     if (p >= cb && p <= cb + 8) {
-                        const c128 v = Vs[(8 * p + 2 * t + h) + (8 * cb + g) * BT_LDV];
+                        // window row R = 8p+2t+h, reflector c = 8cb+g: inside the parallelogram iff 0 <= R - c < 64
+                        c128 v = cmake(0.0, 0.0);
+                        if ((p != cb || 2 * t + h >= g) && (p != cb + 8 || 2 * t + h < g))
+                            v = Vs[(8 * p + 2 * t + h) + (8 * cb + g) * BT_LDV];
                         // (ar + i ai) * (v.x - i v.y)
                         dmma_p(y1r[c][h], ar, v.x);
                         dmma_p(y1i[c][h], ai, v.x);
@@ -252,7 +295,7 @@ __device__ __forceinline__ void bt_apply_step(const c128* __restrict__ Vs, const
             for (int ci = co; ci < NB; ++ci)
 #pragma unroll
                 for (int h = 0; h < 2; ++h) {
-                    const c128 tt = Ts[(8 * (cb0 + co) + g) + (8 * (cb0 + ci) + 2 * t + h) * BT_LDT];
+                    const c128 tt = Ts[s * GS * (GS + 1) + (8 * co + g) + (8 * ci + 2 * t + h) * (GS + 1)];
                     const double ar = ar1[ci][h], ai = ai1[ci][h], nai = -ai;
                     dmma_p(yr[co], ar, tt.x);
                     dmma_p(yi[co], ai, tt.x);
@@ -269,7 +312,9 @@ __device__ __forceinline__ void bt_apply_step(const c128* __restrict__ Vs, const
                 const double ar = yr[c][h], ai = yi[c][h], nai = -ai;
 #pragma unroll
                 for (int p = cb; p <= cb + 8; ++p) {
-                    const c128 v = Vs[(8 * p + g) + (8 * cb + 2 * t + h) * BT_LDV];
+                    c128 v = cmake(0.0, 0.0);
+                    if ((p != cb || g >= 2 * t + h) && (p != cb + 8 || g < 2 * t + h))
+                        v = Vs[(8 * p + g) + (8 * cb + 2 * t + h) * BT_LDV];
                     dmma_p(zr[p], ar, v.x);
                     dmma_p(zi[p], ai, v.x);
                     dmma_p(zr[p], nai, v.y);
@@ -288,86 +333,100 @@ __device__ __forceinline__ void bt_apply_step(const c128* __restrict__ Vs, const
     }
 }
 
+// Stage producer state (uniform over warp 0; only lane 0 touches shared/global memory).
+struct BtProducer {
+    uint32_t it;       // stages produced so far
+    int pass, slab, k, nk;
+    bool done;
+};
+
 template <int GS>
 __global__ void __launch_bounds__(BT_NT, 1) bt_sweep_kernel(const BtSweepArgs a) {
     extern __shared__ __align__(128) unsigned char bt_raw[];
     c128* Vring = reinterpret_cast<c128*>(bt_raw);
+    constexpr int BT_STAGES = bt_stages(GS), BT_TSZ = bt_tsz(GS);
     c128* Tring = Vring + (size_t)BT_STAGES * BT_VS;
-    BtHeader* hdr = reinterpret_cast<BtHeader*>(Tring + (size_t)BT_STAGES * BT_TS);
+    c128* Zstage = Tring + (size_t)BT_STAGES * BT_TSZ;
+    BtHeader* hdr = reinterpret_cast<BtHeader*>(Zstage + (size_t)BT_CWARPS * BT_ZS);
     uint64_t* full = reinterpret_cast<uint64_t*>(hdr + BT_STAGES);
     uint64_t* empty = full + BT_STAGES;
+    uint64_t* zfull = empty + BT_STAGES;          // one per warp
 
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
-    for (int idx = tid; idx < BT_STAGES * (BT_VS + BT_TS); idx += BT_NT) Vring[idx] = cmake(0.0, 0.0);
+    for (int idx = tid; idx < BT_STAGES * (BT_VS + BT_TSZ) + BT_CWARPS * BT_ZS; idx += BT_NT) Vring[idx] = cmake(0.0, 0.0);
     if (tid == 0) {
         for (int s = 0; s < BT_STAGES; ++s) { mbar_init(&full[s], 1); mbar_init(&empty[s], BT_CWARPS); }
+        for (int w = 0; w < BT_CWARPS; ++w) mbar_init(&zfull[w], 1);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
     __syncthreads();
 
     const int N = a.N;
-    if (warp == BT_CWARPS) {
-        // =============================== producer warp (one lane)
-        if (lane != 0) return;
-        uint32_t it = 0;
-        const unsigned long long total = (unsigned long long)a.npass * a.nslabs;
-        for (;;) {
-            const unsigned long long u = atomicAdd(a.unit_counter, 1ULL);
+    const unsigned long long units_per_group = (unsigned long long)a.nslabs * a.chain;
+    const unsigned long long ngroups = (unsigned long long)((a.npass + a.chain - 1) / a.chain);
+    const unsigned long long total = ngroups * units_per_group;
+
+    BtProducer pr;
+    pr.it = 0; pr.pass = 0; pr.slab = 0; pr.k = 0; pr.nk = 0; pr.done = false;
+
+    // produce one stage (warp 0 only; all lanes keep the state, lane 0 acts)
+    auto produce = [&]() {
+        if (pr.done) return;
+        while (pr.k == pr.nk) {
+            unsigned long long u = 0;
+            if (lane == 0) u = atomicAdd(a.unit_counter, 1ULL);
+            u = __shfl_sync(0xffffffffu, u, 0);
             if (u >= total) {
-                const int slot = it % BT_STAGES;
-                mbar_wait(&empty[slot], ((it / BT_STAGES) & 1) ^ 1);
-                hdr[slot].flags = 4;
-                mbar_arrive(&full[slot]);
-                break;
+                const int slot = pr.it % BT_STAGES;
+                if (lane == 0) {
+                    mbar_wait(&empty[slot], ((pr.it / BT_STAGES) & 1) ^ 1);
+                    hdr[slot].flags = 4;
+                    mbar_arrive(&full[slot]);
+                }
+                ++pr.it;
+                pr.done = true;
+                return;
             }
-            const int round = (int)(u / a.nslabs);
-            const int pass = a.npass - 1 - round;
-            const int slab = (int)(u % a.nslabs);
-            const int j0 = pass * BT_P;
-            // all eight warps of the unit (pass+1, slab) must have stored their rows
-            while (*(volatile int*)(a.slab_done + slab) < BT_CWARPS * round) {}
-            __threadfence();
-            const int nk = (N - 1 - j0 + BT_B - 1) / BT_B;
-            const c128* Tn = a.Tneg + (size_t)a.pass_off[pass] * BT_TS;
-            for (int k = 0; k < nk; ++k, ++it) {
-                const int slot = it % BT_STAGES;
-                mbar_wait(&empty[slot], ((it / BT_STAGES) & 1) ^ 1);
+            const unsigned long long g = u / units_per_group, rem = u % units_per_group;
+            pr.slab = (int)(rem / a.chain);
+            pr.pass = a.npass - 1 - (int)(g * a.chain + rem % a.chain);
+            pr.k = 0;
+            pr.nk = (pr.pass >= 0) ? (N - 1 - pr.pass * BT_P + BT_B - 1) / BT_B : 0;   // padding units of the last group are empty
+        }
+        const int slot = pr.it % BT_STAGES;
+        {
+            const int j0 = pr.pass * BT_P, k = pr.k;
+            if (lane == 0) {
+                mbar_wait(&empty[slot], ((pr.it / BT_STAGES) & 1) ^ 1);
                 BtHeader hh;
-                hh.j0 = j0; hh.k = k; hh.slab = slab;
-                hh.flags = (k == 0 ? 1 : 0) | (k == nk - 1 ? 2 : 0);
+                hh.j0 = j0; hh.k = k; hh.slab = pr.slab; hh.pass = pr.pass;
+                hh.flags = (k == 0 ? 1 : 0) | (k == pr.nk - 1 ? 2 : 0);
+                hh.nk_pred = (pr.pass + 1 < a.npass) ? (N - 1 - (pr.pass + 1) * BT_P + BT_B - 1) / BT_B : 0;
+                hh.pad0 = hh.pad1 = 0;
                 hdr[slot] = hh;
-                uint32_t bytes = BT_TS * sizeof(c128);
-                c128* Vs = Vring + (size_t)slot * BT_VS;
-#pragma unroll 1
-                for (int t = 0; t < BT_P; ++t) {
-                    const int j = j0 + t;
-                    const int len = min(BT_B, N - (j + 1 + k * BT_B));
-                    if (j <= N - 2 && len > 0) bytes += len * (int)sizeof(c128);
-                }
-                mbar_arrive_expect_tx(&full[slot], bytes);
-#pragma unroll 1
-                for (int t = 0; t < BT_P; ++t) {
-                    const int j = j0 + t;
-                    const int len = min(BT_B, N - (j + 1 + k * BT_B));
-                    if (j <= N - 2 && len > 0) {
-                        const int64_t voff = (int64_t)j * (N - 1) - (int64_t)j * (j - 1) / 2;
-                        bulk_g2s(Vs + t * (BT_LDV + 1), a.V2 + voff + (int64_t)k * BT_B, len * (int)sizeof(c128), &full[slot]);
-                    }
-                }
-                bulk_g2s(Tring + (size_t)slot * BT_TS, Tn + (size_t)k * BT_TS, BT_TS * sizeof(c128), &full[slot]);
+                mbar_arrive_expect_tx(&full[slot], (uint32_t)((BT_VS + BT_TSZ) * sizeof(c128)));
+                // the 32 reflectors of (pass, k) are one contiguous, zero-padded 32 KB tile; -T is 32 (GS+1) elements
+                const int64_t stage = a.pass_off[pr.pass] + k;
+                bulk_g2s(Vring + (size_t)slot * BT_VS, a.V2 + stage * BT_VS, BT_VS * sizeof(c128), &full[slot]);
+                bulk_g2s(Tring + (size_t)slot * BT_TSZ, a.Tneg + stage * BT_TS, BT_TSZ * sizeof(c128), &full[slot]);
             }
         }
-        return;
-    }
+        ++pr.it;
+        ++pr.k;
+    };
 
-    // =================================== consumer warps
+    if (warp == 0)
+        for (int s = 0; s < BT_STAGES - 1; ++s) produce();
+
     const int g = lane >> 2, t = lane & 3;
     double zr[BT_NBLK][2], zi[BT_NBLK][2];
 #pragma unroll
     for (int p = 0; p < BT_NBLK; ++p) zr[p][0] = zr[p][1] = zi[p][0] = zi[p][1] = 0.0;
+    uint32_t zphase = 0;
 
     for (uint32_t it = 0;; ++it) {
+        if (warp == 0) produce();                 // stage it + STAGES - 1
         const int slot = it % BT_STAGES;
         mbar_wait(&full[slot], (it / BT_STAGES) & 1);
         const BtHeader hh = hdr[slot];
@@ -377,7 +436,20 @@ __global__ void __launch_bounds__(BT_NT, 1) bt_sweep_kernel(const BtSweepArgs a)
         const bool colok = col < a.nev;
         c128* Zc = a.Z + (int64_t)col * a.ldz;
         const int nrows = N - R0;                 // valid rows of the window (>= 1)
+        const bool last = (hh.flags & 2) != 0;
+        int* myprog = a.prog + ((size_t)hh.pass * a.nslabs + hh.slab) * BT_CWARPS + warp;
+        const int* predprog = myprog + (size_t)a.nslabs * BT_CWARPS;     // same warp of unit (pass+1, slab)
+        c128* Zs = Zstage + (size_t)warp * BT_ZS;
+        const int mycol = hh.slab * BT_SLAB + warp * 8 + lane;           // column served by lanes 0..7 in bulk copies
+        const bool issuer = lane < 8 && mycol < a.nev;
         if (hh.flags & 1) {
+            // first step of the unit: the whole 96-row window straight from global memory.  Its last rows are
+            // finalised by step 0 of the predecessor.
+            if (hh.nk_pred > 0) {
+                if (lane == 0) while (bt_ld_acquire(predprog) < 1) {}
+                __syncwarp();
+                asm volatile("fence.proxy.async.global;" ::: "memory");  // rows were written through the async proxy
+            }
 #pragma unroll
             for (int p = 0; p < BT_NBLK; ++p)
 #pragma unroll
@@ -389,12 +461,34 @@ __global__ void __launch_bounds__(BT_NT, 1) bt_sweep_kernel(const BtSweepArgs a)
                 }
         }
         const c128* Vs = Vring + (size_t)slot * BT_VS;
-        const c128* Ts = Tring + (size_t)slot * BT_TS;
-        bt_apply_step<GS>(Vs, Ts, zr, zi, g, t, nrows < BT_WR, nrows);
+        const c128* Ts = Tring + (size_t)slot * BT_TSZ;
+        constexpr int NSUB = BT_P / GS;
+        bt_apply_step<GS, NSUB - 1, NSUB - 1>(Vs, Ts, zr, zi, g, t, nrows < BT_WR, nrows);
+        // ---- prefetch the 64 rows that enter the window after this step: one 1-D bulk copy per column into
+        //      this warp's staging tile (no registers, no LSU queue entries held across the step).  They are
+        //      finalised by step k+1 of the predecessor.
+        const int nin = last ? 0 : min(BT_B, nrows - BT_WR);          // incoming rows (may be <= 0 near the end)
+        if (nin > 0) {
+            if (hh.nk_pred > 0) {
+                const int need = min(hh.k + 2, hh.nk_pred);
+                if (lane == 0) while (bt_ld_acquire(predprog) < need) {}
+            }
+            if (lane < 8) bulk_wait_read<0>();                         // the tile's previous bulk stores have read it
+            if (lane == 0) {
+                int ncol = min(8, a.nev - (hh.slab * BT_SLAB + warp * 8));
+                if (ncol < 0) ncol = 0;
+                mbar_arrive_expect_tx(&zfull[warp], (uint32_t)(ncol * nin) * (uint32_t)sizeof(c128));
+            }
+            __syncwarp();
+            if (issuer)
+                bulk_g2s(Zs + lane * BT_LDZ, a.Z + (int64_t)mycol * a.ldz + R0 + BT_WR, (uint32_t)nin * (uint32_t)sizeof(c128),
+                         &zfull[warp]);
+        }
+        if constexpr (NSUB > 1) bt_apply_step<GS, (NSUB > 1 ? NSUB - 2 : 0), 0>(Vs, Ts, zr, zi, g, t, nrows < BT_WR, nrows);
         __syncwarp();
         if (lane == 0) mbar_arrive(&empty[slot]);
-        if (hh.flags & 2) {
-            // last step of the unit: store the whole window
+        if (last) {
+            // last step of the unit: store the whole window (generic stores), then publish the unit as complete
 #pragma unroll
             for (int p = 0; p < BT_NBLK; ++p)
 #pragma unroll
@@ -402,31 +496,54 @@ __global__ void __launch_bounds__(BT_NT, 1) bt_sweep_kernel(const BtSweepArgs a)
                     const int w = 8 * p + 2 * t + e;
                     if (colok && w < nrows) Zc[R0 + w] = cmake(zr[p][e], zi[p][e]);
                 }
-            __threadfence();
+            if (lane < 8) bulk_wait<0>();
             __syncwarp();
-            if (lane == 0) atomicAdd(a.slab_done + hh.slab, 1);
+            if (lane == 0) bt_st_release(myprog, hh.k + 1);
+            __syncwarp();
         } else {
-            // store the finished top 64 rows, slide the window, fetch the next 64 rows
+            // exchange through the staging tile: every lane takes its incoming element and leaves the finished
+            // one at the same address; then the 64 finished rows leave by one bulk store per column
+            if (nin > 0) {
+                mbar_wait(&zfull[warp], zphase);
+                zphase ^= 1;
+            } else {
+                if (lane < 8) bulk_wait_read<0>();                     // no prefetch this step: the tile may still be read
+                __syncwarp();
+            }
+            c128 vin[8][2];
 #pragma unroll
             for (int p = 0; p < 8; ++p)
 #pragma unroll
                 for (int e = 0; e < 2; ++e) {
                     const int w = 8 * p + 2 * t + e;
-                    if (colok && w < nrows) Zc[R0 + w] = cmake(zr[p][e], zi[p][e]);
+                    c128* q = Zs + g * BT_LDZ + w;
+                    vin[p][e] = (w < nin) ? *q : cmake(0.0, 0.0);
+                    *q = cmake(zr[p][e], zi[p][e]);
                 }
 #pragma unroll
             for (int p = 0; p < BT_NBLK - 8; ++p)
 #pragma unroll
                 for (int e = 0; e < 2; ++e) { zr[p][e] = zr[p + 8][e]; zi[p][e] = zi[p + 8][e]; }
 #pragma unroll
-            for (int p = BT_NBLK - 8; p < BT_NBLK; ++p)
+            for (int p = 0; p < 8; ++p)
 #pragma unroll
                 for (int e = 0; e < 2; ++e) {
-                    const int w = 8 * p + 2 * t + e + BT_B;       // row offset from the old R0
-                    c128 v = cmake(0.0, 0.0);
-                    if (colok && w < nrows) v = __ldcg(Zc + R0 + w);
-                    zr[p][e] = v.x; zi[p][e] = v.y;
+                    zr[BT_NBLK - 8 + p][e] = colok ? vin[p][e].x : 0.0;
+                    zi[BT_NBLK - 8 + p][e] = colok ? vin[p][e].y : 0.0;
                 }
+            asm volatile("fence.proxy.async.shared::cta;" ::: "memory");     // the tile was written by generic stores
+            __syncwarp();
+            if (issuer) bulk_s2g(a.Z + (int64_t)mycol * a.ldz + R0, Zs + lane * BT_LDZ, BT_B * (uint32_t)sizeof(c128));
+            if (lane < 8) {
+                bulk_commit();
+                bulk_wait<1>();                                     // the stores of step k-1 are complete
+            }
+            __syncwarp();
+            // ---- publish the previous step
+            if (hh.k > 0 && (hh.k & 1) == 0) {                      // every second step: the release fence is not free
+                if (lane == 0) bt_st_release(myprog, hh.k);
+                __syncwarp();
+            }
         }
     }
 }
@@ -436,14 +553,22 @@ static int bt_launch_sweep(eigh_handle_s* h, const BtSweepArgs& a, cudaStream_t 
     auto kern = bt_sweep_kernel<GS>;
     static bool attr = false;
     if (!attr) {
-        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)BT_SMEM);
+        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bt_smem(GS));
         if (e != cudaSuccess) return 1000 + (int)e;
         attr = true;
     }
     int grid = h->num_sms;
     const long long units = (long long)a.npass * a.nslabs;
     if (grid > units) grid = (int)units;
-    kern<<<grid, BT_NT, BT_SMEM, s>>>(a);
+    kern<<<grid, BT_NT, bt_smem(GS), s>>>(a);
+    ++h->launches;
+    const cudaError_t e = cudaGetLastError();
+    return e != cudaSuccess ? 1000 + (int)e : 0;
+}
+
+int launch_pass_off(eigh_handle_s* h, cudaStream_t s) {
+    const int npass = (int)bt_npass(h->N);
+    bt_pass_off_kernel<<<1, 32, 0, s>>>((int)h->N, npass, ws_ptr<int64_t>(h, h->plan.pass_off));
     ++h->launches;
     const cudaError_t e = cudaGetLastError();
     return e != cudaSuccess ? 1000 + (int)e : 0;
@@ -462,9 +587,9 @@ int phase_backtransform_band(eigh_handle_s* h, const double* Qt, int64_t ldq, c1
     char* scr = ws_ptr<char>(h, pl.bt) + round_up((size_t)h->b * nev * sizeof(c128), 256);
     int64_t* pass_off = reinterpret_cast<int64_t*>(scr);
     unsigned long long* counter = reinterpret_cast<unsigned long long*>(pass_off + npass + 4);
-    int* slab_done = reinterpret_cast<int*>(counter + 2);
+    int* prog = reinterpret_cast<int*>(counter + 2);
     c128* Tneg = ws_ptr<c128>(h, pl.btT);
-    EIGH_CUDA_OK(cudaMemsetAsync(counter, 0, 16 + (size_t)(nslabs + 8) * sizeof(int), s));
+    EIGH_CUDA_OK(cudaMemsetAsync(counter, 0, 16 + (size_t)npass * nslabs * BT_CWARPS * sizeof(int), s));
     bt_pass_off_kernel<<<1, 32, 0, s>>>(N, npass, pass_off);
     const int kmax = (int)bc_kmax(h);
     int gs = h->g;
@@ -480,7 +605,9 @@ int phase_backtransform_band(eigh_handle_s* h, const double* Qt, int64_t ldq, c1
     h->launches += 2;
     BtSweepArgs a;
     a.Z = Z; a.ldz = ldz; a.N = N; a.nev = nev; a.V2 = ws_ptr<c128>(h, pl.V2); a.Tneg = Tneg; a.pass_off = pass_off;
-    a.npass = npass; a.nslabs = nslabs; a.unit_counter = counter; a.slab_done = slab_done;
+    a.npass = npass; a.nslabs = nslabs; a.unit_counter = counter; a.prog = prog;
+    a.chain = h->bt_chain > 0 ? h->bt_chain : (N >= 16384 ? 4 : 1);
+    if (a.chain > npass) a.chain = npass;
     int rc;
     if (gs == 8) rc = bt_launch_sweep<8>(h, a, s);
     else if (gs == 16) rc = bt_launch_sweep<16>(h, a, s);

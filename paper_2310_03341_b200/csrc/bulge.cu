@@ -15,7 +15,8 @@
 // cooperatively so that every CTA is resident (the wait chain always ends at a running sweep).
 //
 // Reflectors (LAPACK zlarfg convention, H = I - tau v v^H, v_0 = 1 stored explicitly) are packed:
-// V2[off(j) + row - j - 1], off(j) = j (N-1) - j (j-1)/2; tau of (sweep j, step k) at tau2[j kmax + k].
+// tile-major (eigh_internal.h): v_{j,k}[i] at V2[((pass_off[j/32] + k) 32 + j%32) 64 + i], zero padded;
+// tau of (sweep j, step k) at tau2[j kmax + k].
 #include <limits.h>
 
 #include "eigh_internal.h"
@@ -32,6 +33,7 @@ struct BcArgs {
     c128* band; int64_t ldab;
     int N;
     c128* V2;
+    const int64_t* pass_off;
     c128* tau2;       // [N][kmax]: tau of reflector (sweep j, step k) at tau2[j*kmax + k]
     int kmax;
     int* progress;    // [N], zero on entry
@@ -293,7 +295,7 @@ __device__ __forceinline__ bool bc_step(BcSmem& sm, const BcStepCtx& t, int r0, 
         }
     }
     if (q == 0) {
-        if (FULL || r < len2) t.Vj[r0 + BC_B + r] = vnr;
+        t.Vj[(int64_t)(k + 1) * (32 * BC_B) + r] = vnr;          // zero beyond len2
         sm.vs[r] = vnr;
     }
     if (t.tid == 0) t.tau2j[k + 1] = taun;
@@ -331,8 +333,7 @@ __global__ void __launch_bounds__(BC_NT + 32, 1) bulge_chase_kernel(const BcArgs
     int hb = 0;
 
     for (int j = blockIdx.x; j <= N - 2; j += gridDim.x) {
-        const int64_t voff = (int64_t)j * (N - 1) - (int64_t)j * (j - 1) / 2;   // packed column j
-        t.Vj = a.V2 + voff - j - 1;                  // Vj[row] for row in j+1..N-1
+        t.Vj = a.V2 + ((a.pass_off[j >> 5] * 32 + (j & 31)) * BC_B);     // reflector (j, k) at Vj[k * 2048 + i]
         t.tau2j = a.tau2 + (int64_t)j * a.kmax;
         if (tid == 0) bc_poll(a.progress, j - 1, 2);
         bc_sync_compute();
@@ -348,8 +349,8 @@ __global__ void __launch_bounds__(BC_NT + 32, 1) bulge_chase_kernel(const BcArgs
             if (q == 0) {
                 if (r < len) {
                     colj[1 + r] = (r == 0) ? cmake(beta, 0.0) : cmake(0.0, 0.0);
-                    t.Vj[j + 1 + r] = vr;
                 }
+                t.Vj[r] = vr;                                 // zero beyond len
                 sm.vs[r] = vr;
             }
             if (tid == 0) t.tau2j[0] = tau;
@@ -393,6 +394,12 @@ int phase_band_to_tridiag(eigh_handle_s* h, c128* band, int64_t ldab, double* d,
     int* progress = ws_ptr<int>(h, pl.bc_progress);
     double* sgn = ws_ptr<double>(h, pl.sgn);
     EIGH_CUDA_OK(cudaMemsetAsync(progress, 0, (size_t)(N + 8) * sizeof(int), s));
+    // reflector slots that no (sweep, step) writes (short sweeps of a pass, sweeps beyond N-2) must read as zero
+    EIGH_CUDA_OK(cudaMemsetAsync(ws_ptr<c128>(h, pl.V2), 0, (size_t)v2_total_stages(N) * 32 * 64 * sizeof(c128), s));
+    {
+        const int rc = launch_pass_off(h, s);
+        if (rc) return rc;
+    }
     if (N >= 2) {
         const size_t smem = sizeof(BcSmem);
         static bool attr = false;
@@ -408,6 +415,7 @@ int phase_band_to_tridiag(eigh_handle_s* h, c128* band, int64_t ldab, double* d,
         if (G > N - 1) G = N - 1;
         BcArgs a;
         a.band = band; a.ldab = ldab; a.N = N; a.V2 = ws_ptr<c128>(h, pl.V2); a.progress = progress;
+        a.pass_off = ws_ptr<int64_t>(h, pl.pass_off);
         a.tau2 = ws_ptr<c128>(h, pl.tau2); a.kmax = (int)bc_kmax(h);
         void* kargs[] = {(void*)&a};
         EIGH_CUDA_OK(cudaLaunchCooperativeKernel((void*)bulge_chase_kernel, dim3(G), dim3(BC_NT + 32), kargs, smem, s));

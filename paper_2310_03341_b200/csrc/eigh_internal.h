@@ -19,7 +19,8 @@ struct WsPlan {
     size_t Vp, VT, X;                          // (N x b) c128 panel temporaries (Vp = explicit V)
     size_t small;                              // b x b c128 scratch (Gram, S) x 4
     size_t panel_sync;                         // cooperative panel kernel: counters + partial dots
-    size_t V2;                                 // packed stage-2 reflectors, N(N-1)/2 c128
+    size_t V2;                                 // stage-2 reflectors, tile-major: [(pass, k) stage][32 sweeps][64] c128
+    size_t pass_off;                           // int64[npass + 1]: first stage of every pass of 32 sweeps
     size_t tau2;                               // stage-2 taus, N x kmax c128 (kmax = bc_kmax)
     size_t bc_progress;                        // bulge chasing progress counters (N int32)
     size_t d, e, sgn;                          // tridiagonal (N doubles each) and row signs
@@ -41,6 +42,7 @@ struct eigh_handle_s {
     int g;          // WY group size for S4a
     int leaf;       // D&C leaf size
     int p4b_merge;  // panels per WY block in S4b
+    int bt_chain;   // S4a: consecutive passes of one slab scheduled back to back (0 = auto)
     int bc_grid;    // S2: CTAs of the bulge-chasing kernel (0 = all that are co-resident)
     int64_t ldab;   // band storage leading dimension
     void* ws;
@@ -68,6 +70,18 @@ static inline int64_t bc_kmax(const eigh_handle_s* h) {
     const int64_t k = (h->N - 1 + h->b - 1) / h->b;
     return k < 1 ? 1 : k;
 }
+
+// Stage-2 reflector storage.  Sweeps are grouped into passes of 32; (pass p, step k) is one stage of 32
+// reflectors x 64 elements, zero padded, stored contiguously (so that S4a fetches a stage with ONE bulk copy):
+//   v_{j,k}[i]  at  V2[((pass_off[j / 32] + k) * 32 + j % 32) * 64 + i],   pass p has ceil((N-1-32p)/64) stages.
+static inline int64_t v2_npass(int64_t N) { return N >= 2 ? (N - 1 + 31) / 32 : 0; }
+static inline int64_t v2_pass_stages(int64_t N, int64_t p) { return (N - 1 - 32 * p + 63) / 64; }
+static inline int64_t v2_total_stages(int64_t N) {
+    int64_t st = 0;
+    for (int64_t p = 0; p < v2_npass(N); ++p) st += v2_pass_stages(N, p);
+    return st;
+}
+int launch_pass_off(eigh_handle_s* h, cudaStream_t s);   // fills plan.pass_off (bt_band.cu)
 
 // phase drivers (each enqueues on `s`; returns 0 or an error code)
 int phase_reduce_to_band(eigh_handle_s* h, c128* A, int64_t lda, c128* band, int64_t ldab, cudaStream_t s);
