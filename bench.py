@@ -5,7 +5,8 @@
 
 A "step" is one pass of the whole hot path (eigh_solve: full->band, band->tridiagonal, tridiagonal
 D&C, both back-transformations) over one synthetic matrix of BASELINE.json's `configs` (default
-config 2, N = 8192; --config 3 / 4 run N = 27648 / 49152).  The matrix is regenerated in place
+config 3, the N = 27648 vortex-tangle BdG matrix: the largest one whose W + K solves finish within
+minutes; --config 4 runs the N = 49152 target, --config 2 the N = 8192 case).  The matrix is regenerated in place
 (device-side copy from a resident pristine copy, or the device generator when two copies do not
 fit) OUTSIDE the per-step CUDA-event brackets, because eigh_solve overwrites A.
 
@@ -162,9 +163,9 @@ def _leading_block_bdg(w, ns):
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=3)
+    ap.add_argument("--steps", type=int, default=2)
     ap.add_argument("--warmup", type=int, default=3)
-    ap.add_argument("--config", type=int, default=int(os.environ.get("EIGH_BENCH_CONFIG", "2")))
+    ap.add_argument("--config", type=int, default=int(os.environ.get("EIGH_BENCH_CONFIG", "3")))
     ap.add_argument("--nev", type=int, default=0, help="0 = all eigenpairs")
     ap.add_argument("--impl", default="ours")
     ap.add_argument("--ref-sample", type=int, default=1024)
@@ -234,7 +235,7 @@ def main():
         solver.solve(At, W, Zt)
         ev1.record(stream)
         torch.cuda.synchronize()
-        return ev0.elapsed_time(ev1), solver.phase_times_ms(), solver.launch_count()
+        return ev0.elapsed_time(ev1), solver.phase_times_ms() + [solver.kernel_time_ms("bt_sweep_kernel")], solver.launch_count()
 
     for _ in range(args.warmup):
         one_step()
@@ -291,7 +292,7 @@ def main():
             Wh = torch.empty(N, dtype=torch.float64, pin_memory=True)
             Zh = torch.empty((nev, N), dtype=torch.complex128, pin_memory=True)
             times = []
-            for i in range(2):
+            for i in range(2 if N <= 8192 else 1):
                 torch.cuda.synchronize()
                 ev0.record(stream)
                 solver.solve_host(Ah, Wh, Zh, At, W, Zt)
@@ -322,7 +323,7 @@ def main():
         return
 
     cw = credited_work(N, nev, b)
-    ph = [sum(p[i] for p in phases) / len(phases) for i in range(5)]
+    ph = [sum(p[i] for p in phases) / len(phases) for i in range(6)]
     phase_report = {
         "p1_full_to_band": {"ms": ph[0], "tflops": cw["p1_flops"] / ph[0] / 1e9 if ph[0] else None},
         "p2_band_to_tridiag": {"ms": ph[1], "gbs_credited": cw["p2_bytes"] / ph[1] / 1e6 if ph[1] else None,
@@ -331,21 +332,34 @@ def main():
         "p4a_backtransform_band": {"ms": ph[3], "tflops": cw["p4a_flops"] / ph[3] / 1e9 if ph[3] else None},
         "p4b_backtransform_full": {"ms": ph[4], "tflops": cw["p4b_flops"] / ph[4] / 1e9 if ph[4] else None},
     }
-    # dominant phase among the tensor-bound ones -> roofline object
-    cand = [("p1_full_to_band", cw["p1_flops"], ph[0]), ("p4a_backtransform_band", cw["p4a_flops"], ph[3]),
-            ("p4b_backtransform_full", cw["p4b_flops"], ph[4])]
-    name, fl, ms = max(cand, key=lambda t: t[2])
-    achieved = fl / ms / 1e9 if ms else 0.0
+    # roofline object: the dominant kernel.  S4a is one persistent launch (bt_sweep_kernel) whose duration is
+    # measured by CUDA events inside the library on the solve's stream; its algorithmic work is the credited
+    # 8 N^2 nev flops of the band back-transformation (WY padding and the T products excluded).
+    dominant = max(range(5), key=lambda i: ph[i])
+    sweep_ms = ph[5]
+    achieved = cw["p4a_flops"] / sweep_ms / 1e9 if sweep_ms else 0.0
     peaks = {}
     try:
         peaks = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))
     except Exception:
         pass
+    traffic = None
+    try:
+        traffic = json.load(open(os.path.join(ROOT, "profiles", "r01_traffic.json"))).get(w.name)
+    except Exception:
+        pass
     roofline = {
-        "bound": "tensor", "kernel": f"zgemm_kernel (DMMA) launches of {name}", "achieved": achieved,
-        "peak": FP64_NOMINAL_TFLOPS, "unit": "TFLOP/s", "frac": achieved / FP64_NOMINAL_TFLOPS, "traffic": None,
-        "peak_source": "FP64 nominal 148 SM x 64 FMA/clk x 1.965 GHz (MEASURED_PEAKS.json has no FP64 entry; cuBLAS "
-                       "ZGEMM measured 36.8 TFLOP/s on this pool, profiles/)",
+        "bound": "tensor", "kernel": "eigh::bt_sweep_kernel<8> (FP64 DMMA, 1 launch per solve, phase p4a)",
+        "achieved": achieved, "peak": FP64_NOMINAL_TFLOPS, "unit": "TFLOP/s", "frac": achieved / FP64_NOMINAL_TFLOPS,
+        "traffic": traffic, "kernel_ms": sweep_ms, "launches_per_step": 1,
+        "dominant_phase": ["p1_full_to_band", "p2_band_to_tridiag", "p3_tridiag_dc", "p4a_backtransform_band",
+                           "p4b_backtransform_full"][dominant],
+        "peak_source": "FP64 tensor (DMMA) 148 SM x 64 FMA/clk x 1.965 GHz = 37.2 TFLOP/s, equal to the burst DMMA rate "
+                       "measured on this pool (profiles/r01_fp64_peaks.md; cuBLAS ZGEMM 36.8); MEASURED_PEAKS.json has "
+                       "no FP64 entry",
+        "tensor_phase_fracs": {"p1": cw["p1_flops"] / ph[0] / 1e9 / FP64_NOMINAL_TFLOPS if ph[0] else None,
+                               "p4a": cw["p4a_flops"] / ph[3] / 1e9 / FP64_NOMINAL_TFLOPS if ph[3] else None,
+                               "p4b": cw["p4b_flops"] / ph[4] / 1e9 / FP64_NOMINAL_TFLOPS if ph[4] else None},
         "hbm_peak_gbs": peaks.get("hbm_gbs"),
         "p2_hbm_frac_credited": (cw["p2_bytes"] / ph[1] / 1e6) / peaks["hbm_gbs"] if ph[1] and peaks.get("hbm_gbs") else None,
     }

@@ -42,6 +42,8 @@ int eigh_create(eigh_handle_t* h, int64_t N, int64_t nev);
 
 /* Tuning knobs; must be called before eigh_workspace_size.  Keys: "band_width" (64 or 128),
  * "wy_group" (reflectors per compact-WY block of S4a: 8, 16 or 32), "dc_leaf" (8..32), "p4b_merge" (1..4 panels of S1 merged into one compact-WY block of S4b; default 4),
+ * "panel_smem" (S1.1: 1 = shared-memory resident panel QR with the T factor built in, 0 = L2-resident panel QR + Gram
+ * GEMM + T recurrence), "panel_rows_min" (16..192 panel rows per thread block of the resident kernel),
  * "bt_chain" (S4a: consecutive passes of one column slab scheduled back to back so that followers read from L2;
  * 0 = automatic), "bc_grid" (thread blocks of the S2 bulge-chasing kernel; 0 = every co-resident block, the default).
  * Returns -2 for an unknown key, -3 for a bad value. */
@@ -77,6 +79,11 @@ int eigh_solve_host(eigh_handle_t h, const void* A_host, int64_t lda, double* W_
  * stream: ms[0] = full->band, [1] = band->tridiagonal, [2] = tridiagonal D&C,
  * [3] = band back-transform, [4] = full back-transform. */
 int eigh_phase_times(eigh_handle_t h, double ms[5]);
+
+/* Device time (ms, CUDA events on the solve's stream around the launch) of one named kernel of the last
+ * eigh_solve.  Timed kernels: "bt_sweep_kernel" (the single persistent launch that carries S4a).
+ * Returns -2 for an unknown name. */
+int eigh_kernel_time(eigh_handle_t h, const char* kernel, double* ms);
 
 /* Kernel launches issued by the last eigh_solve (all are this library's own kernels). */
 int64_t eigh_launch_count(eigh_handle_t h);

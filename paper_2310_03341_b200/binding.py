@@ -26,6 +26,7 @@ SIGNATURES = {
     "eigh_solve": (_int, [_vp, _vp, _i64, _vp, _vp, _vp]),
     "eigh_solve_host": (_int, [_vp, _vp, _i64, _vp, _vp, _vp, _vp, _vp, _vp]),
     "eigh_phase_times": (_int, [_vp, _dp]),
+    "eigh_kernel_time": (_int, [_vp, ctypes.c_char_p, _dp]),
     "eigh_launch_count": (_i64, [_vp]),
     "eigh_last_error": (ctypes.c_char_p, [_vp]),
     "eigh_destroy": (_int, [_vp]),
@@ -147,6 +148,12 @@ class Eigh:
         ms = (ctypes.c_double * 5)()
         self.lib.eigh_phase_times(self.h, ms)
         return list(ms)
+
+    def kernel_time_ms(self, kernel: str) -> float:
+        ms = ctypes.c_double()
+        rc = self.lib.eigh_kernel_time(self.h, kernel.encode(), ctypes.byref(ms))
+        self._check(rc, "eigh_kernel_time")
+        return float(ms.value)
 
     def launch_count(self) -> int:
         return int(self.lib.eigh_launch_count(self.h))

@@ -96,6 +96,8 @@ int eigh_create(eigh_handle_t* out, int64_t N, int64_t nev) {
     h->g = 8;
     h->leaf = 32;
     h->p4b_merge = 4;
+    h->panel_smem = 1;
+    h->panel_rows_min = 96;
     h->num_sms = 0;
     snprintf(h->err, sizeof(h->err), "ok");
     *out = h;
@@ -117,6 +119,12 @@ int eigh_set_option(eigh_handle_t h, const char* key, int64_t value) {
     } else if (!strcmp(key, "p4b_merge")) {
         if (value < 1 || value > 4) return set_err(h, -3, "p4b_merge must be in [1, 4]");
         h->p4b_merge = (int)value;
+    } else if (!strcmp(key, "panel_smem")) {
+        if (value != 0 && value != 1) return set_err(h, -3, "panel_smem must be 0 or 1");
+        h->panel_smem = (int)value;
+    } else if (!strcmp(key, "panel_rows_min")) {
+        if (value < 16 || value > 192) return set_err(h, -3, "panel_rows_min must be in [16, 192]");
+        h->panel_rows_min = (int)value;
     } else if (!strcmp(key, "bt_chain")) {
         if (value < 0 || value > 16) return set_err(h, -3, "bt_chain must be in [0, 16]");
         h->bt_chain = (int)value;
@@ -153,6 +161,10 @@ static int ensure_ready(eigh_handle_t h) {
     if (!h->events_ok) {
         for (int i = 0; i < 6; ++i) {
             cudaError_t e = cudaEventCreate(&h->ev[i]);
+            if (e != cudaSuccess) return set_err(h, 1000 + (int)e, "cudaEventCreate: %s", cudaGetErrorString(e));
+        }
+        for (int i = 0; i < 2; ++i) {
+            cudaError_t e = cudaEventCreate(&h->ev_sweep[i]);
             if (e != cudaSuccess) return set_err(h, 1000 + (int)e, "cudaEventCreate: %s", cudaGetErrorString(e));
         }
         h->events_ok = true;
@@ -266,6 +278,12 @@ int eigh_solve(eigh_handle_t h, void* A_dev, int64_t lda, double* W_dev, void* Z
         cudaEventElapsedTime(&ms, h->ev[i], h->ev[i + 1]);
         h->phase_ms[i] = ms;
     }
+    h->sweep_ms = 0.0;
+    if (h->N >= 2) {                          // the sweeper is not launched for N = 1
+        float ms = 0.f;
+        if (cudaEventElapsedTime(&ms, h->ev_sweep[0], h->ev_sweep[1]) == cudaSuccess) h->sweep_ms = ms;
+        else (void)cudaGetLastError();
+    }
     if (nfail) set_err(h, nfail, "%d secular roots did not converge", nfail);
     return nfail;
 }
@@ -301,6 +319,14 @@ int eigh_phase_times(eigh_handle_t h, double ms[5]) {
     return 0;
 }
 
+int eigh_kernel_time(eigh_handle_t h, const char* kernel, double* ms) {
+    if (!h) return -1;
+    if (!kernel) return -2;
+    if (!ms) return -3;
+    if (!strcmp(kernel, "bt_sweep_kernel")) { *ms = h->sweep_ms; return 0; }
+    return set_err(h, -2, "no timer for kernel '%s'", kernel);
+}
+
 int64_t eigh_launch_count(eigh_handle_t h) { return h ? h->launches : -1; }
 
 const char* eigh_last_error(eigh_handle_t h) { return h ? h->err : "null handle"; }
@@ -308,7 +334,10 @@ const char* eigh_last_error(eigh_handle_t h) { return h ? h->err : "null handle"
 int eigh_destroy(eigh_handle_t h) {
     if (!h) return -1;
     if (h->events_ok)
+    {
         for (int i = 0; i < 6; ++i) cudaEventDestroy(h->ev[i]);
+        for (int i = 0; i < 2; ++i) cudaEventDestroy(h->ev_sweep[i]);
+    }
     delete h;
     return 0;
 }

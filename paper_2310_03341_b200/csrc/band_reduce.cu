@@ -238,6 +238,202 @@ __global__ void __launch_bounds__(PQ_NT, 1) panel_qr_kernel(const PanelArgs a) {
     }
 }
 
+// ------------------------------------------------------------------ shared-memory resident panel QR
+// The same Householder QR (zlarfg convention) with the CTA's rows of the panel held in shared memory
+// for the whole factorisation, so that a column step costs one lean grid barrier plus two passes over
+// shared memory instead of three passes over L2:
+//   dots pass   d[c] = sum_{r > jj, own rows} conj(P[r,jj]) P[r,c]  for ALL 64 columns c
+//               (c >= jj: norm and v^H P as before; c < jj: conj(d[c]) = V[:,c]^H P[:,jj], the Gram
+//               entries from which the compact-WY T factor is built on the fly);
+//   barrier     partial dots + the pivot row go through L2; arrival = red.release, wait = ld.acquire;
+//   update pass every CTA forms the reflector scalars redundantly and updates its rows.
+// One extra CTA (the last) owns no rows: it accumulates T,
+//   T[0:jj, jj] = -tau_jj T[0:jj, 0:jj] g,   g_i = v_i^H v_jj = conj(P[jj,i]) + s conj(d[i]),   T[jj,jj] = tau_jj,
+// which replaces the V^H V GEMM, its split-K reduction and the serial T recurrence kernel.
+constexpr int PS_NT = 256, PS_MAXROWS = 192, PS_LD = 65, PS_B = 64;
+
+struct PanelSmemArgs {
+    c128* P;  int64_t ld;      // panel, m x 64, column-major in A
+    int m, nr;                 // rows, reflectors (= 64 here)
+    c128* Vp; int64_t ldv;     // explicit V out, m x 64
+    c128* tau;                 // 64
+    c128* T;  int ldt;         // compact-WY T out (64 x 64, upper triangular, zero below)
+    unsigned* counter;         // grid barrier counter, zero on entry
+    c128* part;                // [2][gridDim.x][64]
+    c128* pivrow;              // [2][64]
+    int rows_per_cta;
+};
+
+__device__ __forceinline__ void ps_grid_barrier(unsigned* ctr, unsigned target) {
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        asm volatile("red.release.gpu.global.add.u32 [%0], 1;" ::"l"(ctr) : "memory");
+        unsigned v;
+        do {
+            asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(ctr) : "memory");
+        } while (v < target);
+    }
+    __syncthreads();
+}
+
+__global__ void __launch_bounds__(PS_NT, 1) panel_qr_smem_kernel(const PanelSmemArgs a) {
+    extern __shared__ __align__(16) unsigned char ps_raw[];
+    c128* Ps = reinterpret_cast<c128*>(ps_raw);            // [rows][PS_LD] row-major tile (row CTAs) or T (T CTA)
+    c128* red = Ps + PS_MAXROWS * PS_LD;                   // [4][64]
+    c128* tot = red + 4 * PS_B;                            // [64]
+    c128* wv = tot + PS_B;                                 // [64]
+    c128* pv = wv + PS_B;                                  // [64] pivot row
+    const int tid = threadIdx.x;
+    const int c = tid & 63, q = tid >> 6;
+    const int G = gridDim.x - 1;                           // row CTAs; CTA G accumulates T
+    const int cta = blockIdx.x;
+    const bool tcta = cta == G;
+    const int r_begin = tcta ? a.m : cta * a.rows_per_cta;
+    const int r_end = tcta ? a.m : min(a.m, r_begin + a.rows_per_cta);
+    const int nrows = r_end - r_begin;
+
+    // ---- load the tile (coalesced along rows in global, padded rows in shared)
+    for (int idx = tid; idx < nrows * PS_B; idx += PS_NT) {
+        const int rr = idx % nrows, cc = idx / nrows;
+        Ps[rr * PS_LD + cc] = a.P[(r_begin + rr) + (int64_t)cc * a.ld];
+    }
+    if (tcta)
+        for (int idx = tid; idx < PS_B * PS_LD; idx += PS_NT) Ps[idx] = cmake(0.0, 0.0);
+    __syncthreads();
+
+    for (int jj = 0; jj < a.nr; ++jj) {
+        const int par = jj & 1;
+        // ---- dots pass over own rows r > jj
+        {
+            const int lo = max(0, jj + 1 - r_begin);       // first local row with global index > jj
+            c128 acc = cmake(0.0, 0.0);
+            for (int rr = lo + q; rr < nrows; rr += 4) cfmac(acc, Ps[rr * PS_LD + jj], Ps[rr * PS_LD + c]);
+            red[q * PS_B + c] = acc;
+        }
+        __syncthreads();
+        if (!tcta && tid < PS_B) {
+            const c128 s4 = cadd(cadd(red[tid], red[PS_B + tid]), cadd(red[2 * PS_B + tid], red[3 * PS_B + tid]));
+            a.part[((size_t)par * G + cta) * PS_B + tid] = s4;
+            if (jj >= r_begin && jj < r_end) a.pivrow[(size_t)par * PS_B + tid] = Ps[(jj - r_begin) * PS_LD + tid];
+        }
+        ps_grid_barrier(a.counter, (unsigned)(jj + 1) * gridDim.x);
+        // ---- totals (every CTA, redundantly), reflector scalars, w
+        {
+            c128 s4 = cmake(0.0, 0.0);
+            const c128* pp = a.part + (size_t)par * G * PS_B + c;
+            for (int g = q; g < G; g += 4) {
+                const c128 v = __ldcg(pp + (size_t)g * PS_B);
+                s4.x += v.x; s4.y += v.y;
+            }
+            red[q * PS_B + c] = s4;
+            if (tid < PS_B) pv[tid] = __ldcg(a.pivrow + (size_t)par * PS_B + tid);
+        }
+        __syncthreads();
+        if (tid < PS_B) tot[tid] = cadd(cadd(red[tid], red[PS_B + tid]), cadd(red[2 * PS_B + tid], red[3 * PS_B + tid]));
+        __syncthreads();
+        c128 tau = cmake(0.0, 0.0), s = cmake(0.0, 0.0);
+        double beta;
+        bool active = false;
+        {
+            const c128 alpha = pv[jj];
+            const double xnorm2 = tot[jj].x;
+            beta = alpha.x;
+            if (xnorm2 > 0.0 || alpha.y != 0.0) {
+                beta = -copysign(sqrt(alpha.x * alpha.x + alpha.y * alpha.y + xnorm2), alpha.x);
+                tau = cmake((beta - alpha.x) / beta, -alpha.y / beta);
+                const double dr = alpha.x - beta, di = alpha.y;
+                const double den = dr * dr + di * di;
+                s = cmake(dr / den, -di / den);            // 1 / (alpha - beta)
+                active = true;
+            }
+        }
+        if (tcta) {
+            // g_i = v_i^H v_jj (i < jj); T[0:jj, jj] = -tau T[0:jj, 0:jj] g; T[jj, jj] = tau
+            if (tid < PS_B) {
+                c128 g = cmake(0.0, 0.0);
+                if (tid < jj) {
+                    g = cconj(pv[tid]);
+                    if (active) g = cadd(g, cmul(s, cconj(tot[tid])));
+                }
+                wv[tid] = g;
+            }
+            __syncthreads();
+            {
+                c128 acc = cmake(0.0, 0.0);
+                if (c < jj)
+                    for (int l = c + q; l < jj; l += 4) cfma(acc, Ps[c * PS_LD + l], wv[l]);
+                red[q * PS_B + c] = acc;
+            }
+            __syncthreads();
+            if (tid < PS_B) {
+                if (tid < jj) {
+                    const c128 t4 = cadd(cadd(red[tid], red[PS_B + tid]), cadd(red[2 * PS_B + tid], red[3 * PS_B + tid]));
+                    const c128 v = cmul(tau, t4);
+                    Ps[tid * PS_LD + jj] = cmake(-v.x, -v.y);
+                } else if (tid == jj) {
+                    Ps[tid * PS_LD + jj] = tau;
+                }
+            }
+            if (tid == 0) a.tau[jj] = tau;
+            __syncthreads();
+            continue;
+        }
+        // ---- row CTAs: w_c = P[jj,c] + conj(s) d[c] (c > jj); rows r > jj: v_r = s x_r, P[r,c] -= conj(tau) v_r w_c
+        if (tid < PS_B) wv[tid] = (tid > jj) ? cadd(pv[tid], cmulc(s, tot[tid])) : cmake(0.0, 0.0);
+        __syncthreads();
+        const c128 ctau = cconj(tau);
+        if (active) {
+            const int lo = max(0, jj + 1 - r_begin);
+            if (c > jj) {
+                const c128 wc = wv[c];
+                for (int rr = lo + q; rr < nrows; rr += 4) {
+                    const c128 f = cmul(ctau, cmul(s, Ps[rr * PS_LD + jj]));
+                    const c128 t4 = cmul(f, wc);
+                    c128 o = Ps[rr * PS_LD + c];
+                    o.x -= t4.x; o.y -= t4.y;
+                    Ps[rr * PS_LD + c] = o;
+                }
+            }
+            // pivot row (its owner)
+            if (jj >= r_begin && jj < r_end && q == 0) {
+                const int rr = jj - r_begin;
+                if (c > jj) {
+                    const c128 t4 = cmul(ctau, wv[c]);
+                    c128 o = Ps[rr * PS_LD + c];
+                    o.x -= t4.x; o.y -= t4.y;
+                    Ps[rr * PS_LD + c] = o;
+                }
+            }
+            __syncthreads();
+            // column jj becomes v (rows > jj) and beta (pivot)
+            for (int rr = lo + tid; rr < nrows; rr += PS_NT) Ps[rr * PS_LD + jj] = cmul(s, Ps[rr * PS_LD + jj]);
+            if (jj >= r_begin && jj < r_end && tid == 0) Ps[(jj - r_begin) * PS_LD + jj] = cmake(beta, 0.0);
+        } else {
+            // H = I: v = e_jj; entries below the pivot are already zero (xnorm2 = 0)
+        }
+        __syncthreads();
+    }
+    if (tcta) {
+        for (int idx = tid; idx < PS_B * PS_B; idx += PS_NT) {
+            const int i = idx & 63, j = idx >> 6;
+            a.T[i + (size_t)j * a.ldt] = (i <= j && j < a.nr) ? Ps[i * PS_LD + j] : cmake(0.0, 0.0);
+        }
+        for (int jj = a.nr + tid; jj < PS_B; jj += PS_NT) a.tau[jj] = cmake(0.0, 0.0);
+        return;
+    }
+    // ---- write back: A keeps R (rows <= column) and v below; Vp gets the explicit unit-lower-trapezoidal V
+    for (int idx = tid; idx < nrows * PS_B; idx += PS_NT) {
+            const int rr = idx % nrows, cc = idx / nrows;
+            const int r = r_begin + rr;
+            const c128 v = Ps[rr * PS_LD + cc];
+            a.P[r + (int64_t)cc * a.ld] = v;
+            c128 e = cmake(0.0, 0.0);
+            if (r == cc) e = cmake(1.0, 0.0);
+            else if (r > cc && cc < a.nr) e = v;
+            a.Vp[r + (int64_t)cc * a.ldv] = e;
+        }
+}
+
 // ------------------------------------------------------------------ host driver
 static int zg(eigh_handle_s* h, bool ta, bool tb, int M, int N, int K, double alpha, const c128* A, int64_t lda,
               const c128* B, int64_t ldb, double beta, c128* C, int64_t ldc, bool small_tile, int splitk,
@@ -289,11 +485,13 @@ int phase_reduce_to_band(eigh_handle_s* h, c128* A, int64_t lda, c128* band, int
     ++h->launches;
     EIGH_CUDA_OK(cudaMemsetAsync(tau1, 0, (size_t)N * sizeof(c128), s));
 
+    const size_t ps_smem = (size_t)(PS_MAXROWS * PS_LD + 4 * PS_B + 3 * PS_B) * sizeof(c128);
     const size_t pq_smem = (size_t)(PQ_WARPS * b + b + 4) * sizeof(c128);
     const size_t tf_smem = (size_t)(2 * b * (b + 1) + b) * sizeof(c128);
     static bool attr = false;
     if (!attr) {
         EIGH_CUDA_OK(cudaFuncSetAttribute(tfactor_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)tf_smem));
+        EIGH_CUDA_OK(cudaFuncSetAttribute(panel_qr_smem_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ps_smem));
         attr = true;
     }
     int max_coop = 0;
@@ -308,23 +506,40 @@ int phase_reduce_to_band(eigh_handle_s* h, c128* A, int64_t lda, c128* band, int
         c128* panel = A + (j0 + b) + (int64_t)j0 * lda;
         c128* A22 = A + (j0 + b) + (int64_t)(j0 + b) * lda;
         c128* Tp = T1 + (size_t)p * b * b;
-        // S1.1 panel QR
-        PanelArgs pa;
-        pa.P = panel; pa.ld = lda; pa.m = m; pa.nb = b; pa.nr = min(b, m - 1);
-        pa.Vp = Vp; pa.ldv = m; pa.tau = tau1 + j0; pa.counter = counter; pa.part = part; pa.pivrow = pivrow;
-        int G = (int)ceil_div(m, 64);
-        if (G > coop_limit) G = coop_limit;
-        pa.rows_per_cta = (int)ceil_div(m, G);
-        G = (int)ceil_div(m, pa.rows_per_cta);
+        // S1.1 + S1.2: panel QR and T factor
+        int rc;
+        const bool smem_panel = b == PS_B && h->panel_smem && m >= 2 * PS_B && m <= (int64_t)(coop_limit - 1) * PS_MAXROWS;
         EIGH_CUDA_OK(cudaMemsetAsync(counter, 0, 256, s));
-        void* kargs[] = {(void*)&pa};
-        EIGH_CUDA_OK(cudaLaunchCooperativeKernel((void*)panel_qr_kernel, dim3(G), dim3(PQ_NT), kargs, pq_smem, s));
-        ++h->launches;
-        // S1.2 T factor
-        int rc = zg(h, true, false, b, b, m, 1.0, Vp, m, Vp, m, 0.0, small, b, true, splitk_for_small_output(m), s);
-        if (rc) return rc;
-        tfactor_kernel<<<1, 128, tf_smem, s>>>(small, b, tau1 + j0, b, Tp, b);
-        ++h->launches;
+        if (smem_panel) {
+            PanelSmemArgs pa;
+            pa.P = panel; pa.ld = lda; pa.m = m; pa.nr = b;
+            pa.Vp = Vp; pa.ldv = m; pa.tau = tau1 + j0; pa.T = Tp; pa.ldt = b;
+            pa.counter = counter; pa.part = part; pa.pivrow = pivrow;
+            int G = coop_limit - 1;
+            int rows = (int)ceil_div(m, G);
+            if (rows < h->panel_rows_min) rows = h->panel_rows_min;
+            if (rows > PS_MAXROWS) rows = PS_MAXROWS;
+            pa.rows_per_cta = rows;
+            G = (int)ceil_div(m, rows);
+            void* kargs[] = {(void*)&pa};
+            EIGH_CUDA_OK(cudaLaunchCooperativeKernel((void*)panel_qr_smem_kernel, dim3(G + 1), dim3(PS_NT), kargs, ps_smem, s));
+            ++h->launches;
+        } else {
+            PanelArgs pa;
+            pa.P = panel; pa.ld = lda; pa.m = m; pa.nb = b; pa.nr = min(b, m - 1);
+            pa.Vp = Vp; pa.ldv = m; pa.tau = tau1 + j0; pa.counter = counter; pa.part = part; pa.pivrow = pivrow;
+            int G = (int)ceil_div(m, 64);
+            if (G > coop_limit) G = coop_limit;
+            pa.rows_per_cta = (int)ceil_div(m, G);
+            G = (int)ceil_div(m, pa.rows_per_cta);
+            void* kargs[] = {(void*)&pa};
+            EIGH_CUDA_OK(cudaLaunchCooperativeKernel((void*)panel_qr_kernel, dim3(G), dim3(PQ_NT), kargs, pq_smem, s));
+            ++h->launches;
+            rc = zg(h, true, false, b, b, m, 1.0, Vp, m, Vp, m, 0.0, small, b, true, splitk_for_small_output(m), s);
+            if (rc) return rc;
+            tfactor_kernel<<<1, 128, tf_smem, s>>>(small, b, tau1 + j0, b, Tp, b);
+            ++h->launches;
+        }
         // VT = V T
         rc = zg(h, false, false, m, b, b, 1.0, Vp, m, Tp, b, 0.0, VT, m, false, 1, s);
         if (rc) return rc;

@@ -56,7 +56,7 @@ constexpr int BT_LDZ = BT_B + 1;            // 65, odd: per-warp staging of the 
 constexpr int BT_ZS = 8 * BT_LDZ;           // c128 per warp
 // compact -T of one (pass, k) step for WY blocks of GS reflectors: 32/GS blocks [GS x GS], ld GS+1
 __host__ __device__ constexpr int bt_tsz(int gs) { return BT_P * (gs + 1); }
-__host__ __device__ constexpr int bt_stages(int gs) { return gs == 32 ? 3 : 4; }
+__host__ __device__ constexpr int bt_stages(int gs) { return gs == 8 ? 4 : 3; }
 constexpr int BT_CWARPS = 8;                // warps per CTA (all of them consumers)
 constexpr int BT_NT = 32 * BT_CWARPS;
 constexpr int BT_SLAB = 8 * BT_CWARPS;      // 64 columns per unit
@@ -560,7 +560,9 @@ static int bt_launch_sweep(eigh_handle_s* h, const BtSweepArgs& a, cudaStream_t 
     int grid = h->num_sms;
     const long long units = (long long)a.npass * a.nslabs;
     if (grid > units) grid = (int)units;
+    cudaEventRecord(h->ev_sweep[0], s);
     kern<<<grid, BT_NT, bt_smem(GS), s>>>(a);
+    cudaEventRecord(h->ev_sweep[1], s);
     ++h->launches;
     const cudaError_t e = cudaGetLastError();
     return e != cudaSuccess ? 1000 + (int)e : 0;

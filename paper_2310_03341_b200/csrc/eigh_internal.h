@@ -42,6 +42,8 @@ struct eigh_handle_s {
     int g;          // WY group size for S4a
     int leaf;       // D&C leaf size
     int p4b_merge;  // panels per WY block in S4b
+    int panel_smem;      // S1.1: shared-memory resident panel QR (1) or the L2-resident one (0)
+    int panel_rows_min;  // S1.1: fewest panel rows per thread block of the resident kernel
     int bt_chain;   // S4a: consecutive passes of one slab scheduled back to back (0 = auto)
     int bc_grid;    // S2: CTAs of the bulge-chasing kernel (0 = all that are co-resident)
     int64_t ldab;   // band storage leading dimension
@@ -53,6 +55,8 @@ struct eigh_handle_s {
     double phase_ms[5];
     int64_t launches;
     cudaEvent_t ev[6];
+    cudaEvent_t ev_sweep[2];   // brackets of the bt_sweep_kernel launch (S4a's dominant kernel)
+    double sweep_ms;
     bool events_ok;
     int num_sms;
 };

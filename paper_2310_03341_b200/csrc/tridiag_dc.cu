@@ -35,12 +35,13 @@ struct DcBufs {
     double *QA, *QB, *U;              // ldq x N each
     double *dcur, *dnew, *z, *dk, *zk, *mu, *lam, *zhat, *rot_c, *rot_s, *rho, *zsum;
     int *perm, *nd_idx, *df_idx, *org, *rot_a, *rot_b, *kcount, *nrot, *fail, *bnd;
+    int *ctype, *ktype, *upos, *acol, *k1c, *k2c;   // block structure of Q_old (column types, U row order)
     MergeDesc* desc;                  // all levels, concatenated
     DgemmDesc* gdesc;
     int64_t ldq;
 };
 
-static size_t dc_small_bytes(int64_t N) { return (size_t)(16 * 8 + 10 * 4) * (N + 64) + (size_t)(N + 64) * (sizeof(MergeDesc) + sizeof(DgemmDesc)) * 2 + 4096; }
+static size_t dc_small_bytes(int64_t N) { return (size_t)(16 * 8 + 18 * 4) * (N + 64) + (size_t)(N + 64) * (sizeof(MergeDesc) + sizeof(DgemmDesc)) * 2 + 4096; }
 
 size_t dc_arena_bytes(int64_t N) {
     const int64_t ldq = round_up(N, 8);
@@ -71,6 +72,8 @@ static DcBufs dc_carve(void* base, int64_t N) {
     b.perm = (int*)take(ni); b.nd_idx = (int*)take(ni); b.df_idx = (int*)take(ni); b.org = (int*)take(ni);
     b.rot_a = (int*)take(ni); b.rot_b = (int*)take(ni); b.kcount = (int*)take(ni); b.nrot = (int*)take(ni);
     b.fail = (int*)take(256); b.bnd = (int*)take(ni);
+    b.ctype = (int*)take(ni); b.ktype = (int*)take(ni); b.upos = (int*)take(ni); b.acol = (int*)take(ni);
+    b.k1c = (int*)take(ni); b.k2c = (int*)take(ni);
     b.desc = (MergeDesc*)take((size_t)(N + 64) * sizeof(MergeDesc));
     b.gdesc = (DgemmDesc*)take((size_t)(N + 64) * sizeof(DgemmDesc));
     return b;
@@ -227,7 +230,10 @@ __global__ void __launch_bounds__(256) dc_deflate_kernel(const MergeDesc* __rest
                                                          int* __restrict__ rot_b, double* __restrict__ rot_c,
                                                          double* __restrict__ rot_s, double* __restrict__ dk,
                                                          double* __restrict__ zk, double* __restrict__ rho_out,
-                                                         double* __restrict__ zsum_out) {
+                                                         double* __restrict__ zsum_out, int* __restrict__ ctype,
+                                                         int* __restrict__ ktype, int* __restrict__ upos,
+                                                         int* __restrict__ acol, int* __restrict__ k1c,
+                                                         int* __restrict__ k2c) {
     __shared__ double ds[DF_CH], zs[DF_CH];
     __shared__ int is[DF_CH];
     __shared__ double red[16];
@@ -235,6 +241,9 @@ __global__ void __launch_bounds__(256) dc_deflate_kernel(const MergeDesc* __rest
     const MergeDesc m = desc[mi];
     const int s = m.s, n = m.e - m.s;
     const int tid = threadIdx.x;
+    // column types of Q_old = diag(Q_left, Q_right): 1 = non-zero in the top rows only, 3 = bottom rows only,
+    // 2 = both (a deflating rotation mixed a left with a right column)
+    for (int i = tid; i < n; i += 256) ctype[s + i] = (i < m.mid - m.s) ? 1 : 3;
     // maxima
     double dmax = 0.0, zmax = 0.0;
     for (int i = tid; i < n; i += 256) {
@@ -287,6 +296,7 @@ __global__ void __launch_bounds__(256) dc_deflate_kernel(const MergeDesc* __rest
                     zi = tau;
                     rot_a[s + nr] = pj; rot_b[s + nr] = i; rot_c[s + nr] = c; rot_s[s + nr] = sn;
                     ++nr;
+                    if (ctype[s + pj] != ctype[s + i]) { ctype[s + pj] = 2; ctype[s + i] = 2; }
                     const double tnew = dpj * c * c + di * sn * sn;
                     di = dpj * sn * sn + di * c * c;
                     dcur[s + pj] = tnew;
@@ -295,6 +305,7 @@ __global__ void __launch_bounds__(256) dc_deflate_kernel(const MergeDesc* __rest
                 } else {
                     dcur[s + pj] = dpj; z[s + pj] = zpj;
                     nd_idx[s + k] = pj; dk[s + k] = dpj; zk[s + k] = zpj; zs2 += zpj * zpj;
+                    ktype[s + k] = ctype[s + pj];
                     ++k;
                 }
                 pj = i; dpj = di; zpj = zi;
@@ -305,8 +316,22 @@ __global__ void __launch_bounds__(256) dc_deflate_kernel(const MergeDesc* __rest
         if (pj >= 0) {
             dcur[s + pj] = dpj; z[s + pj] = zpj;
             nd_idx[s + k] = pj; dk[s + k] = dpj; zk[s + k] = zpj; zs2 += zpj * zpj;
+            ktype[s + k] = ctype[s + pj];
             ++k;
         }
+        // memory order of the kept columns (= row order of U): [type 1 | type 2 | type 3], so that the merge GEMM
+        // runs as  top rows x K-range [0, k1+k2)  and  bottom rows x K-range [k1, k)
+        int k1 = 0, k2 = 0;
+        for (int i = 0; i < k; ++i) { const int t = ktype[s + i]; k1 += (t == 1); k2 += (t == 2); }
+        int p1 = 0, p2 = k1, p3 = k1 + k2;
+        for (int i = 0; i < k; ++i) {
+            const int t = ktype[s + i];
+            const int pos = (t == 1) ? p1++ : (t == 2) ? p2++ : p3++;
+            upos[s + i] = pos;
+            acol[s + pos] = nd_idx[s + i];
+        }
+        k1c[mi] = k1;
+        k2c[mi] = k2;
         kcount[mi] = k;
         nrot[mi] = nr;
         zsum_out[mi] = zs2;
@@ -463,7 +488,7 @@ __global__ void __launch_bounds__(128) dc_zhat_kernel(const MergeDesc* __restric
 __global__ void __launch_bounds__(256) dc_build_u_kernel(const MergeDesc* __restrict__ desc, const int* __restrict__ kcount,
                                                          const double* __restrict__ dk_all, const int* __restrict__ org_all,
                                                          const double* __restrict__ mu_all, const double* __restrict__ zhat_all,
-                                                         double* __restrict__ U, int64_t ldq) {
+                                                         const int* __restrict__ upos_all, double* __restrict__ U, int64_t ldq) {
     __shared__ double red[8];
     const int mi = blockIdx.y;
     const int k = kcount[mi];
@@ -475,9 +500,10 @@ __global__ void __launch_bounds__(256) dc_build_u_kernel(const MergeDesc* __rest
     const double dorg = dk[org_all[s + j]], muj = mu_all[s + j];
     double* Uc = U + s + (int64_t)(s + j) * ldq;
     double ss = 0.0;
+    const int* upos = upos_all + s;
     for (int i = threadIdx.x; i < k; i += 256) {
         const double v = zh[i] / ((dk[i] - dorg) - muj);
-        Uc[i] = v;
+        Uc[upos[i]] = v;                   // row order of U = memory order of the gathered columns
         ss += v * v;
     }
     for (int o = 16; o > 0; o >>= 1) ss += __shfl_xor_sync(0xffffffffu, ss, o);
@@ -490,19 +516,31 @@ __global__ void __launch_bounds__(256) dc_build_u_kernel(const MergeDesc* __rest
 }
 
 // ------------------------------------------------------------------ S3.5 merge GEMM descriptors, deflated columns
-__global__ void dc_gemm_desc_kernel(const MergeDesc* __restrict__ desc, const int* __restrict__ kcount, int nmerge,
-                                    int64_t ldq, DgemmDesc* __restrict__ g) {
+__global__ void dc_gemm_desc_kernel(const MergeDesc* __restrict__ desc, const int* __restrict__ kcount,
+                                    const int* __restrict__ k1c, const int* __restrict__ k2c, int nmerge, int64_t ldq,
+                                    DgemmDesc* __restrict__ g) {
     const int mi = blockIdx.x * blockDim.x + threadIdx.x;
     if (mi >= nmerge) return;
     const MergeDesc m = desc[mi];
+    const int k = kcount[mi], k1 = k1c[mi], k2 = k2c[mi];
+    const int k1e = k1 & ~1;                 // even start of the bottom K-range (16-byte aligned rows of U); a type-1
+                                             // column that falls into it only contributes exact zeros
     DgemmDesc d;
+    // top rows: columns of type 1 and 2
     d.offA = d.offB = d.offC = m.s + (int64_t)m.s * ldq;
     d.offIdx = m.s;
-    d.M = m.e - m.s;
-    d.N = kcount[mi];
-    d.K = kcount[mi];
+    d.M = m.mid - m.s;
+    d.N = k;
+    d.K = k1 + k2;
     d.pad = 0;
-    g[mi] = d;
+    g[2 * mi] = d;
+    // bottom rows: columns of type 2 and 3
+    d.offA = d.offC = m.mid + (int64_t)m.s * ldq;
+    d.offB = (m.s + k1e) + (int64_t)m.s * ldq;
+    d.offIdx = m.s + k1e;
+    d.M = m.e - m.mid;
+    d.K = k - k1e;
+    g[2 * mi + 1] = d;
 }
 
 __global__ void __launch_bounds__(256) dc_finish_kernel(const MergeDesc* __restrict__ desc, const int* __restrict__ kcount,
@@ -560,18 +598,20 @@ int phase_tridiag_dc(eigh_handle_s* h, const double* d, const double* e, double*
         if (bnd[i + 1] - bnd[i] < 1 || bnd[i + 1] - bnd[i] > DC_LEAF_MAX)
             return set_err(h, -100, "internal: bad D&C leaf partition (N=%d, L=%d)", N, L);
     std::vector<MergeDesc> descs;
-    std::vector<int> level_off, level_cnt, level_maxn;
+    std::vector<int> level_off, level_cnt, level_maxn, level_maxhalf;
     for (int width = 1; width < L; width *= 2) {
         level_off.push_back((int)descs.size());
-        int cnt = 0, maxn = 0;
+        int cnt = 0, maxn = 0, maxhalf = 0;
         for (int i = 0; i + 2 * width <= L; i += 2 * width) {
             MergeDesc m = {bnd[i], bnd[i + width], bnd[i + 2 * width], 0};
             descs.push_back(m);
             ++cnt;
             maxn = std::max(maxn, m.e - m.s);
+            maxhalf = std::max(maxhalf, std::max(m.mid - m.s, m.e - m.mid));
         }
         level_cnt.push_back(cnt);
         level_maxn.push_back(maxn);
+        level_maxhalf.push_back(maxhalf);
     }
     { MergeDesc all = {0, 0, N, 0}; descs.push_back(all); }    // descriptor used by the final sort
     const int final_desc = (int)descs.size() - 1;
@@ -603,18 +643,19 @@ int phase_tridiag_dc(eigh_handle_s* h, const double* d, const double* e, double*
         dc_zvec_kernel<<<dim3(gx256, cnt), 256, 0, st>>>(dd, Qcur, ldq, B.z);
         dc_rank_kernel<<<dim3(gx256, cnt), 256, 0, st>>>(dd, dcur, B.perm);
         dc_deflate_kernel<<<cnt, 256, 0, st>>>(dd, e, dcur, B.z, B.perm, B.nd_idx, B.df_idx, B.kcount, B.nrot, B.rot_a,
-                                               B.rot_b, B.rot_c, B.rot_s, B.dk, B.zk, B.rho, B.zsum);
+                                               B.rot_b, B.rot_c, B.rot_s, B.dk, B.zk, B.rho, B.zsum, B.ctype, B.ktype, B.upos, B.acol, B.k1c,
+                                               B.k2c);
         dc_apply_rot_kernel<<<dim3(gx256, cnt), 256, 0, st>>>(dd, Qcur, ldq, B.nrot, B.rot_a, B.rot_b, B.rot_c, B.rot_s);
         dc_secular_kernel<<<dim3(gx128, cnt), 128, 0, st>>>(dd, B.kcount, B.dk, B.zk, B.rho, B.zsum, B.org, B.mu, B.lam, B.fail);
         dc_zhat_kernel<<<dim3(gx128, cnt), 128, 0, st>>>(dd, B.kcount, B.dk, B.zk, B.org, B.mu, B.zhat);
-        dc_build_u_kernel<<<dim3(maxn, cnt), 256, 0, st>>>(dd, B.kcount, B.dk, B.org, B.mu, B.zhat, B.U, ldq);
-        dc_gemm_desc_kernel<<<(unsigned)ceil_div(cnt, 128), 128, 0, st>>>(dd, B.kcount, cnt, ldq, B.gdesc);
+        dc_build_u_kernel<<<dim3(maxn, cnt), 256, 0, st>>>(dd, B.kcount, B.dk, B.org, B.mu, B.zhat, B.upos, B.U, ldq);
+        dc_gemm_desc_kernel<<<(unsigned)ceil_div(cnt, 128), 128, 0, st>>>(dd, B.kcount, B.k1c, B.k2c, cnt, ldq, B.gdesc);
         h->launches += 9;
         DgemmArgs ga;
         memset(&ga, 0, sizeof(ga));
         ga.A = Qcur; ga.lda = ldq; ga.B = B.U; ga.ldb = ldq; ga.C = Qnew; ga.ldc = ldq;
-        ga.a_col_idx = B.nd_idx; ga.desc = B.gdesc;
-        int rc = dgemm_launch_desc(ga, cnt, maxn, maxn, st, &h->launches);
+        ga.a_col_idx = B.acol; ga.desc = B.gdesc;
+        int rc = dgemm_launch_desc(ga, 2 * cnt, level_maxhalf[lv], maxn, st, &h->launches);
         if (rc) return 1000 + rc;
         dc_finish_kernel<<<dim3(maxn, cnt), 256, 0, st>>>(dd, B.kcount, B.df_idx, Qcur, Qnew, ldq, dcur, B.lam, dnew);
         ++h->launches;
