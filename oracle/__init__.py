@@ -4,7 +4,7 @@ Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl refere
 legs may import this package.  paper_2310_03341_b200 never does.
 """
 from .oracle import (build, eigh, eigh_ld, tridiagonalise, tridiag_ql, tridiag_ql_ld,
-                     num_threads)
+                     num_threads, sturm_count)
 
 __all__ = ["build", "eigh", "eigh_ld", "tridiagonalise", "tridiag_ql", "tridiag_ql_ld",
-           "num_threads"]
+           "num_threads", "sturm_count"]

@@ -117,3 +117,27 @@ def tridiag_ql(d, e, vectors: bool = True):
 
 def tridiag_ql_ld(d, e, vectors: bool = True):
     return _tql(d, e, vectors, "_ld")
+
+
+def sturm_count(d, e, sigma):
+    """Number of eigenvalues of the real symmetric tridiagonal T = tridiag(d, e) that are < sigma
+    (Sylvester's law of inertia on the LDL^T pivots of T - sigma I; Golub & Van Loan 8.4.1 /
+    SURVEY.md 8(c) "Sturm-count spot checks").  Plain recurrence
+        q_0 = d_0 - sigma,   q_i = (d_i - sigma) - e_{i-1}^2 / q_{i-1},
+    count = #{i : q_i < 0}; a zero pivot is replaced by a tiny negative number.  `sigma` may be an
+    array: the recurrence is vectorised over the shifts only (O(N) steps, each elementwise).
+    TEST INFRASTRUCTURE ONLY; shares nothing with the CUDA path."""
+    d = np.asarray(d, dtype=np.float64)
+    e = np.asarray(e, dtype=np.float64)
+    sig = np.atleast_1d(np.asarray(sigma, dtype=np.float64))
+    n = d.shape[0]
+    scale = max(np.abs(d).max(initial=0.0), np.abs(e).max(initial=0.0), 1e-300)
+    tiny = scale * np.finfo(np.float64).tiny ** 0.5
+    q = d[0] - sig
+    q = np.where(q == 0.0, -tiny, q)
+    cnt = (q < 0).astype(np.int64)
+    for i in range(1, n):
+        q = (d[i] - sig) - (e[i - 1] * e[i - 1]) / q
+        q = np.where(q == 0.0, -tiny, q)
+        cnt += q < 0
+    return cnt if np.ndim(sigma) else int(cnt[0])

@@ -251,16 +251,20 @@ __device__ __forceinline__ void bt_apply_step(const c128* __restrict__ Vs, const
     for (int s = S_HI; s >= S_LO; --s) {
         const int cb0 = s * NB;
         // ---- Y1 = V^H Z   (m = column of Z, n = reflector, k = row)
-        double y1r[NB][2][2], y1i[NB][2][2];   // [col block][k-step parity h][frag]
+        // 3M form of the complex product (three real DMMAs per complex multiply-add instead of four; the sums
+        // run over all 72 rows before they are combined):  with z = ar + i ai and conj(v) = v.x - i v.y,
+        //   S1 = sum ar v.x,  S2 = sum ai v.y,  S3 = sum (ar + ai)(v.x - v.y);   Re = S1 + S2,  Im = S3 - S1 + S2.
+        double s1[NB][2][2], s2[NB][2][2], s3[NB][2][2];   // [col block][k-step parity h][frag]
 #pragma unroll
         for (int c = 0; c < NB; ++c)
 #pragma unroll
-            for (int h = 0; h < 2; ++h) y1r[c][h][0] = y1r[c][h][1] = y1i[c][h][0] = y1i[c][h][1] = 0.0;
+            for (int h = 0; h < 2; ++h)
+                s1[c][h][0] = s1[c][h][1] = s2[c][h][0] = s2[c][h][1] = s3[c][h][0] = s3[c][h][1] = 0.0;
 #pragma unroll
         for (int p = cb0; p < cb0 + NB + 8; ++p) {
 #pragma unroll
             for (int h = 0; h < 2; ++h) {
-                const double ar = zr[p][h], ai = zi[p][h], nar = -ar;
+                const double ar = zr[p][h], ai = zi[p][h], as = ar + ai;
 #pragma unroll
                 for (int c = 0; c < NB; ++c) {
                     const int cb = cb0 + c;
@@ -269,11 +273,9 @@ __device__ __forceinline__ void bt_apply_step(const c128* __restrict__ Vs, const
                         c128 v = cmake(0.0, 0.0);
                         if ((p != cb || 2 * t + h >= g) && (p != cb + 8 || 2 * t + h < g))
                             v = Vs[(8 * p + 2 * t + h) + (8 * cb + g) * BT_LDV];
-                        // (ar + i ai) * (v.x - i v.y)
-                        dmma_p(y1r[c][h], ar, v.x);
-                        dmma_p(y1i[c][h], ai, v.x);
-                        dmma_p(y1r[c][h], ai, v.y);
-                        dmma_p(y1i[c][h], nar, v.y);
+                        dmma_p(s1[c][h], ar, v.x);
+                        dmma_p(s2[c][h], ai, v.y);
+                        dmma_p(s3[c][h], as, v.x - v.y);
                     }
                 }
             }
@@ -283,8 +285,9 @@ __device__ __forceinline__ void bt_apply_step(const c128* __restrict__ Vs, const
         for (int c = 0; c < NB; ++c)
 #pragma unroll
             for (int e = 0; e < 2; ++e) {
-                ar1[c][e] = y1r[c][0][e] + y1r[c][1][e];
-                ai1[c][e] = y1i[c][0][e] + y1i[c][1][e];
+                const double t1 = s1[c][0][e] + s1[c][1][e], t2 = s2[c][0][e] + s2[c][1][e], t3 = s3[c][0][e] + s3[c][1][e];
+                ar1[c][e] = t1 + t2;
+                ai1[c][e] = (t3 - t1) + t2;
             }
         // ---- Y = (-T) Y1   (m = column of Z, n = output reflector, k = input reflector >= output)
         double yr[NB][2], yi[NB][2];

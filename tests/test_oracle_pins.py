@@ -279,3 +279,34 @@ def test_library_cross_check():
     assert np.abs(W - Wn).max() <= 1e-12 * np.abs(Wn).max()
     assert abs(W.sum() - np.trace(H).real) <= 1e-11
     assert abs(np.sum(W ** 2) - np.linalg.norm(H) ** 2) <= 1e-10 * np.linalg.norm(H) ** 2
+
+
+# ----------------------------------------------------------------------------- Sturm count (used by the full-size GPU tests)
+def test_sturm_count_against_closed_forms():
+    """oracle.sturm_count is pinned by spectra known in closed form: the 1-2-1 Toeplitz matrix
+    (lambda_k = 2 - 2 cos(k pi/(n+1))) and the Clement/Kac matrix (integers -(n-1), -(n-3), ..., n-1)."""
+    n = 200
+    d = np.full(n, 2.0)
+    e = np.full(n - 1, -1.0)
+    lam = 2.0 - 2.0 * np.cos(np.arange(1, n + 1) * np.pi / (n + 1))
+    mids = 0.5 * (lam[:-1] + lam[1:])
+    assert np.array_equal(oracle.sturm_count(d, e, mids), np.arange(1, n))
+    assert oracle.sturm_count(d, e, -1.0) == 0 and oracle.sturm_count(d, e, 5.0) == n
+    n = 51
+    i = np.arange(1, n)
+    ek = np.sqrt(i * (n - i))
+    ints = np.arange(-(n - 1), n, 2).astype(float)
+    assert np.array_equal(oracle.sturm_count(np.zeros(n), ek, ints + 0.5), np.arange(1, n + 1))
+    assert np.array_equal(oracle.sturm_count(np.zeros(n), ek, ints - 0.5), np.arange(0, n))
+
+
+def test_sturm_count_matches_oracle_ql_on_random_tridiagonal():
+    rng = np.random.default_rng(7)
+    n = 300
+    d = rng.standard_normal(n)
+    e = rng.standard_normal(n - 1)
+    W = oracle.tridiag_ql(d, e, vectors=False)
+    gaps = np.diff(W)
+    ok = gaps > 1e-8
+    mids = (0.5 * (W[:-1] + W[1:]))[ok]
+    assert np.array_equal(oracle.sturm_count(d, e, mids), (np.arange(1, n))[ok])
