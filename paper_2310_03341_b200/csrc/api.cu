@@ -96,6 +96,7 @@ int eigh_create(eigh_handle_t* out, int64_t N, int64_t nev) {
     h->g = 8;
     h->leaf = 32;
     h->p4b_merge = 4;
+    h->gemm_3m = 1;
     h->panel_smem = 1;
     h->panel_rows_min = 96;
     h->num_sms = 0;
@@ -119,6 +120,9 @@ int eigh_set_option(eigh_handle_t h, const char* key, int64_t value) {
     } else if (!strcmp(key, "p4b_merge")) {
         if (value < 1 || value > 4) return set_err(h, -3, "p4b_merge must be in [1, 4]");
         h->p4b_merge = (int)value;
+    } else if (!strcmp(key, "gemm_3m")) {
+        if (value != 0 && value != 1) return set_err(h, -3, "gemm_3m must be 0 or 1");
+        h->gemm_3m = (int)value;
     } else if (!strcmp(key, "panel_smem")) {
         if (value != 0 && value != 1) return set_err(h, -3, "panel_smem must be 0 or 1");
         h->panel_smem = (int)value;
@@ -156,6 +160,7 @@ int eigh_set_workspace(eigh_handle_t h, void* ws_dev, size_t bytes) {
 
 static int ensure_ready(eigh_handle_t h) {
     if (!h) return -1;
+    g_zgemm_3m = h->gemm_3m != 0;            // process-wide switch of the GEMM engine, set from the handle in use
     if (!h->ws) return set_err(h, -1, "no workspace set (call eigh_set_workspace)");
     if (!h->planned) return set_err(h, -1, "options changed after eigh_set_workspace; call eigh_workspace_size / eigh_set_workspace again");
     if (!h->events_ok) {

@@ -42,6 +42,7 @@ struct eigh_handle_s {
     int g;          // WY group size for S4a
     int leaf;       // D&C leaf size
     int p4b_merge;  // panels per WY block in S4b
+    int gemm_3m;         // complex GEMMs by the 3M method (1) or with four real products (0)
     int panel_smem;      // S1.1: shared-memory resident panel QR (1) or the L2-resident one (0)
     int panel_rows_min;  // S1.1: fewest panel rows per thread block of the resident kernel
     int bt_chain;   // S4a: consecutive passes of one slab scheduled back to back (0 = auto)

@@ -3,10 +3,10 @@
 
 namespace eigh {
 
-template <int WM, int WN, bool TA, bool TB, int MODE, int MINB>
+template <int WM, int WN, bool TA, bool TB, int MODE, int MINB, int NJ = 4, bool M3 = false>
 static int launch_inst(const ZgemmArgs& a, cudaStream_t stream, int64_t* launches) {
-    using Cfg = ZgemmCfg<WM, WN, TA, TB, MODE>;
-    auto kern = zgemm_kernel<WM, WN, TA, TB, MODE, MINB>;
+    using Cfg = ZgemmCfg<WM, WN, TA, TB, MODE, NJ>;
+    auto kern = zgemm_kernel<WM, WN, TA, TB, MODE, MINB, NJ, M3>;
     static bool attr_set = false;
     if (!attr_set) {
         cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize,
@@ -34,10 +34,19 @@ static int launch_inst(const ZgemmArgs& a, cudaStream_t stream, int64_t* launche
 }
 
 bool g_zgemm_big_tiles = false;   // test hook (eigh_k_zgemm lower_only bit 2)
+bool g_zgemm_3m = true;
 
 int zgemm_launch(const ZgemmArgs& a, bool ta, bool tb, int mode, bool small_tile, cudaStream_t stream,
                  int64_t* launches) {
     if (a.M <= 0 || a.N <= 0) return 0;
+    if (g_zgemm_3m && !g_zgemm_big_tiles) {
+        // 3M kernels: CTA tile 64 x 32 (4 warps of 32 x 16), three CTAs per SM
+        if (mode == ZMODE_HEMM) return launch_inst<2, 2, false, false, ZMODE_HEMM, 3, 2, true>(a, stream, launches);
+        if (!ta && !tb) return launch_inst<2, 2, false, false, ZMODE_GEMM, 3, 2, true>(a, stream, launches);
+        if (!ta && tb) return launch_inst<2, 2, false, true, ZMODE_GEMM, 3, 2, true>(a, stream, launches);
+        if (ta && !tb) return launch_inst<2, 2, true, false, ZMODE_GEMM, 3, 2, true>(a, stream, launches);
+        return (int)cudaErrorInvalidValue;
+    }
     if (mode == ZMODE_HEMM) return launch_inst<2, 2, false, false, ZMODE_HEMM, 2>(a, stream, launches);
     // 64x64 tiles with two resident CTAs per SM are the default: measured faster than 128x64 with one
     // CTA per SM in every shape the solver uses (profiles/r01_gemm_shapes.md)

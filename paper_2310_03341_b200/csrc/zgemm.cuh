@@ -33,9 +33,10 @@ constexpr int ZG_BK = 8;
 constexpr int ZG_STAGES = 4;
 constexpr int ZG_KSTRIDE = ZG_BK + 4;   // K-contiguous tiles: stride == 4 (mod 8) 16B-units
 
-template <int WARPS_M, int WARPS_N, bool TA, bool TB, int MODE>
+// NJ = 8-column fragments per warp in N (warp tile 32 x 8 NJ): 4 for the 4-multiplication kernel, 2 for the 3M one
+template <int WARPS_M, int WARPS_N, bool TA, bool TB, int MODE, int NJ = 4>
 struct ZgemmCfg {
-    static constexpr int BM = 32 * WARPS_M, BN = 32 * WARPS_N, NT = 32 * WARPS_M * WARPS_N;
+    static constexpr int BM = 32 * WARPS_M, BN = 8 * NJ * WARPS_N, NT = 32 * WARPS_M * WARPS_N;
     static constexpr int SA_N = BM + 2;                       // M-contiguous A tile: As[k][m]
     static constexpr int SB_C = BN + 2;                       // N-contiguous B tile: Bs[k][n]
     static constexpr int A_N_SIZE = ZG_BK * SA_N, A_C_SIZE = BM * ZG_KSTRIDE;
@@ -89,10 +90,54 @@ __device__ __forceinline__ void zgemm_compute_stage(const c128* __restrict__ As,
     }
 }
 
-template <int WARPS_M, int WARPS_N, bool TA, bool TB, int MODE, int MINB>
+// 3M variant (Karatsuba / "zgemm3m"): three real products per complex multiply-add,
+//   S1 += ar br,  S2 += ai bi,  S3 += (ar + ai)(br + bi);   Re = S1 - S2,  Im = S3 - S1 - S2  (combined once, after the K loop).
+// 25 % fewer DMMAs for two extra DADDs per fragment; normwise error bound of the same order as the conventional
+// product (the imaginary part loses componentwise, not normwise, accuracy).  Warp tile 32 x 8 NJ.
+template <int BM, int BN, int NJ, bool ACT, bool CONJA, bool BCT, bool CONJB>
+__device__ __forceinline__ void zgemm_compute_stage_3m(const c128* __restrict__ As, const c128* __restrict__ Bs,
+                                                       int wm0, int wn0, int g, int t, double (&s1)[4][NJ][2],
+                                                       double (&s2)[4][NJ][2], double (&s3)[4][NJ][2]) {
+    constexpr int SA_N = BM + 2, SB_C = BN + 2;
+#pragma unroll
+    for (int kk = 0; kk < ZG_BK; kk += 4) {
+        double ar[4], ai[4], as[4], br[NJ], bi[NJ], bs[NJ];
+#pragma unroll
+        for (int i = 0; i < 4; ++i) {
+            const int m = wm0 + 8 * i + g;
+            const c128 a = ACT ? As[m * ZG_KSTRIDE + kk + t] : As[(kk + t) * SA_N + m];
+            ar[i] = a.x;
+            ai[i] = CONJA ? -a.y : a.y;
+            as[i] = ar[i] + ai[i];
+        }
+#pragma unroll
+        for (int j = 0; j < NJ; ++j) {
+            const int n = wn0 + 8 * j + g;
+            const c128 b = BCT ? Bs[(kk + t) * SB_C + n] : Bs[n * ZG_KSTRIDE + kk + t];
+            br[j] = b.x;
+            bi[j] = CONJB ? -b.y : b.y;
+            bs[j] = br[j] + bi[j];
+        }
+#pragma unroll
+        for (int i = 0; i < 4; ++i)
+#pragma unroll
+            for (int j = 0; j < NJ; ++j) dmma884p(s1[i][j][0], s1[i][j][1], ar[i], br[j]);
+#pragma unroll
+        for (int i = 0; i < 4; ++i)
+#pragma unroll
+            for (int j = 0; j < NJ; ++j) dmma884p(s2[i][j][0], s2[i][j][1], ai[i], bi[j]);
+#pragma unroll
+        for (int i = 0; i < 4; ++i)
+#pragma unroll
+            for (int j = 0; j < NJ; ++j) dmma884p(s3[i][j][0], s3[i][j][1], as[i], bs[j]);
+    }
+}
+
+template <int WARPS_M, int WARPS_N, bool TA, bool TB, int MODE, int MINB, int NJ = 4, bool M3 = false>
 __global__ void __launch_bounds__(32 * WARPS_M * WARPS_N, MINB) zgemm_kernel(const ZgemmArgs p) {
-    using Cfg = ZgemmCfg<WARPS_M, WARPS_N, TA, TB, MODE>;
+    using Cfg = ZgemmCfg<WARPS_M, WARPS_N, TA, TB, MODE, NJ>;
     constexpr int BM = Cfg::BM, BN = Cfg::BN, NT = Cfg::NT, BK = ZG_BK;
+    static_assert(M3 || NJ == 4, "the 4-multiplication kernel uses 32 x 32 warp tiles");
     extern __shared__ __align__(16) unsigned char zg_smem_raw[];
     c128* smem = reinterpret_cast<c128*>(zg_smem_raw);
 
@@ -101,7 +146,7 @@ __global__ void __launch_bounds__(32 * WARPS_M * WARPS_N, MINB) zgemm_kernel(con
 
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int g = lane >> 2, t = lane & 3;
-    const int wm0 = (warp % WARPS_M) * 32, wn0 = (warp / WARPS_M) * 32;
+    const int wm0 = (warp % WARPS_M) * 32, wn0 = (warp / WARPS_M) * (8 * NJ);
 
     const int nkb1 = (p.K1 + BK - 1) / BK;
     const int nkb2 = (p.A2 != nullptr) ? (p.K2 + BK - 1) / BK : 0;
@@ -110,7 +155,14 @@ __global__ void __launch_bounds__(32 * WARPS_M * WARPS_N, MINB) zgemm_kernel(con
     const int kb_begin = blockIdx.z * per;
     const int kb_end = min(nkb, kb_begin + per);
 
-    double cr[4][4][2], ci[4][4][2];
+    // 4-multiplication kernel: cr, ci.  3M kernel: cr = S1, ci = S3 and s2 = S2 (combined in the epilogue).
+    double cr[4][NJ][2], ci[4][NJ][2], s2[M3 ? 4 : 1][M3 ? NJ : 1][2];
+    if (M3) {
+#pragma unroll
+        for (int i = 0; i < 4; ++i)
+#pragma unroll
+            for (int j = 0; j < NJ; ++j) s2[M3 ? i : 0][M3 ? j : 0][0] = s2[M3 ? i : 0][M3 ? j : 0][1] = 0.0;
+    }
     // beta == +-alpha: start the accumulators at (beta/alpha) C (exact), so that the read of C overlaps
     // the pipeline prologue instead of serialising the epilogue
     const bool preload = (p.splitk == 1) && (p.beta != 0.0) && (p.beta == p.alpha || p.beta == -p.alpha);
@@ -120,21 +172,21 @@ __global__ void __launch_bounds__(32 * WARPS_M * WARPS_N, MINB) zgemm_kernel(con
         for (int i = 0; i < 4; ++i) {
             const int row = m0 + wm0 + 8 * i + g;
 #pragma unroll
-            for (int j = 0; j < 4; ++j)
+            for (int j = 0; j < NJ; ++j)
 #pragma unroll
                 for (int e = 0; e < 2; ++e) {
                     const int col = n0 + wn0 + 8 * j + 2 * t + e;
                     c128 v = cmake(0.0, 0.0);
                     if (row < p.M && col < p.N) v = p.C[row + (int64_t)col * p.ldc];
                     cr[i][j][e] = sg * v.x;
-                    ci[i][j][e] = sg * v.y;
+                    ci[i][j][e] = M3 ? sg * (v.x + v.y) : sg * v.y;      // 3M: Im = S3 - S1 - S2
                 }
         }
     } else {
 #pragma unroll
         for (int i = 0; i < 4; ++i)
 #pragma unroll
-            for (int j = 0; j < 4; ++j) cr[i][j][0] = cr[i][j][1] = ci[i][j][0] = ci[i][j][1] = 0.0;
+            for (int j = 0; j < NJ; ++j) cr[i][j][0] = cr[i][j][1] = ci[i][j][0] = ci[i][j][1] = 0.0;
     }
 
     auto a_ctype = [&](int kb) -> bool {
@@ -216,16 +268,40 @@ __global__ void __launch_bounds__(32 * WARPS_M * WARPS_N, MINB) zgemm_kernel(con
         const int stage = (kb - kb_begin) % ZG_STAGES;
         const c128* As = smem + (size_t)stage * Cfg::STAGE;
         const c128* Bs = As + Cfg::A_STAGE;
-        if (MODE == ZMODE_HEMM) {
-            if (a_ctype(kb))
-                zgemm_compute_stage<BM, BN, true, true, TB, TB>(As, Bs, wm0, wn0, g, t, cr, ci);
-            else
-                zgemm_compute_stage<BM, BN, false, false, TB, TB>(As, Bs, wm0, wn0, g, t, cr, ci);
+        if constexpr (M3) {
+            if (MODE == ZMODE_HEMM) {
+                if (a_ctype(kb))
+                    zgemm_compute_stage_3m<BM, BN, NJ, true, true, TB, TB>(As, Bs, wm0, wn0, g, t, cr, s2, ci);
+                else
+                    zgemm_compute_stage_3m<BM, BN, NJ, false, false, TB, TB>(As, Bs, wm0, wn0, g, t, cr, s2, ci);
+            } else {
+                zgemm_compute_stage_3m<BM, BN, NJ, TA, TA, TB, TB>(As, Bs, wm0, wn0, g, t, cr, s2, ci);
+            }
         } else {
-            zgemm_compute_stage<BM, BN, TA, TA, TB, TB>(As, Bs, wm0, wn0, g, t, cr, ci);
+            if (MODE == ZMODE_HEMM) {
+                if (a_ctype(kb))
+                    zgemm_compute_stage<BM, BN, true, true, TB, TB>(As, Bs, wm0, wn0, g, t, cr, ci);
+                else
+                    zgemm_compute_stage<BM, BN, false, false, TB, TB>(As, Bs, wm0, wn0, g, t, cr, ci);
+            } else {
+                zgemm_compute_stage<BM, BN, TA, TA, TB, TB>(As, Bs, wm0, wn0, g, t, cr, ci);
+            }
         }
     }
     cp_async_wait<0>();
+    if constexpr (M3) {
+        // Re = S1 - S2, Im = S3 - S1 - S2
+#pragma unroll
+        for (int i = 0; i < 4; ++i)
+#pragma unroll
+            for (int j = 0; j < NJ; ++j)
+#pragma unroll
+                for (int e = 0; e < 2; ++e) {
+                    const double a1 = cr[i][j][e], a2 = s2[i][j][e], a3 = ci[i][j][e];
+                    cr[i][j][e] = a1 - a2;
+                    ci[i][j][e] = (a3 - a1) - a2;
+                }
+    }
 
     // epilogue
     if (p.splitk > 1) {
@@ -234,7 +310,7 @@ __global__ void __launch_bounds__(32 * WARPS_M * WARPS_N, MINB) zgemm_kernel(con
         for (int i = 0; i < 4; ++i) {
             const int row = m0 + wm0 + 8 * i + g;
 #pragma unroll
-            for (int j = 0; j < 4; ++j)
+            for (int j = 0; j < NJ; ++j)
 #pragma unroll
                 for (int e = 0; e < 2; ++e) {
                     const int col = n0 + wn0 + 8 * j + 2 * t + e;
@@ -247,7 +323,7 @@ __global__ void __launch_bounds__(32 * WARPS_M * WARPS_N, MINB) zgemm_kernel(con
         for (int i = 0; i < 4; ++i) {
             const int row = m0 + wm0 + 8 * i + g;
 #pragma unroll
-            for (int j = 0; j < 4; ++j)
+            for (int j = 0; j < NJ; ++j)
 #pragma unroll
                 for (int e = 0; e < 2; ++e) {
                     const int col = n0 + wn0 + 8 * j + 2 * t + e;
@@ -296,5 +372,6 @@ static __global__ void zgemm_splitk_reduce_kernel(int M, int N, int splitk, cons
 int zgemm_launch(const ZgemmArgs& a, bool ta, bool tb, int mode, bool small_tile, cudaStream_t stream,
                  int64_t* launches);
 extern bool g_zgemm_big_tiles;
+extern bool g_zgemm_3m;       // 3M kernels (default) or the 4-multiplication ones (option "gemm_3m" = 0)
 
 }  // namespace eigh
