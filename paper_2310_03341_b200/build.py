@@ -12,7 +12,7 @@ OBJ = os.path.join(HERE, "build")
 LIB = os.path.join(HERE, "libeigh_b200.so")
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
-         "-Xcompiler", "-fPIC", "-Xcompiler", "-O2"]
+         "-Xcompiler", "-fPIC", "-Xcompiler", "-O2"] + os.environ.get("EIGH_NVCC_EXTRA", "").split()
 
 
 def _stale(target, deps):

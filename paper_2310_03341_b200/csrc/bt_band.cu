@@ -429,7 +429,6 @@ __global__ void __launch_bounds__(BT_NT, 1) bt_sweep_kernel(const BtSweepArgs a)
     uint32_t zphase = 0;
 
     for (uint32_t it = 0;; ++it) {
-        if (warp == 0) produce();                 // stage it + STAGES - 1
         const int slot = it % BT_STAGES;
         mbar_wait(&full[slot], (it / BT_STAGES) & 1);
         const BtHeader hh = hdr[slot];
@@ -487,7 +486,9 @@ __global__ void __launch_bounds__(BT_NT, 1) bt_sweep_kernel(const BtSweepArgs a)
                 bulk_g2s(Zs + lane * BT_LDZ, a.Z + (int64_t)mycol * a.ldz + R0 + BT_WR, (uint32_t)nin * (uint32_t)sizeof(c128),
                          &zfull[warp]);
         }
-        if constexpr (NSUB > 1) bt_apply_step<GS, (NSUB > 1 ? NSUB - 2 : 0), 0>(Vs, Ts, zr, zi, g, t, nrows < BT_WR, nrows);
+        if constexpr (NSUB > 2) bt_apply_step<GS, (NSUB > 2 ? NSUB - 2 : 0), (NSUB > 2 ? 1 : 0)>(Vs, Ts, zr, zi, g, t, nrows < BT_WR, nrows);
+        if (warp == 0) produce();                 // stage it + STAGES - 1
+        if constexpr (NSUB > 1) bt_apply_step<GS, 0, 0>(Vs, Ts, zr, zi, g, t, nrows < BT_WR, nrows);
         __syncwarp();
         if (lane == 0) mbar_arrive(&empty[slot]);
         if (last) {

@@ -111,10 +111,20 @@ __device__ __forceinline__ void bc_handoff_wait(int odd) {
     else asm volatile("bar.sync 2, %0;" ::"n"(BC_NT + 32) : "memory");
 }
 
+#ifdef BC_PROFILE
+__device__ unsigned long long g_bc_prof[16];
+#define BC_STAMP(i) do { if (t.tid == 0) { const long long now_ = clock64(); atomicAdd(&g_bc_prof[i], (unsigned long long)(now_ - t.last)); t.last = now_; } } while (0)
+#else
+#define BC_STAMP(i) do { } while (0)
+#endif
+
 struct BcStepCtx {
     c128* band; int64_t ldab;
     c128* Vj; c128* tau2j;
     int r, q, rl, lane, warp, tid;
+#ifdef BC_PROFILE
+    mutable long long last;
+#endif
 };
 
 // LAPACK zlarfg on a vector spread over the rows (x = element r, zero for r >= len; all four q lanes of
@@ -164,44 +174,82 @@ __device__ __forceinline__ bool bc_step(BcSmem& sm, const BcStepCtx& t, int r0, 
             if (FULL || (r < len2 && q + 4 * i < len)) sreg[i] = __ldcg(sp + (int64_t)i * 4 * (ldab - 1));
         }
     }
+    BC_STAMP(1);
     cp_async_wait<0>();
     bc_sync_compute();                                   // D landed; vs of this step visible
+    BC_STAMP(2);
     c128 vc[BC_NC];
 #pragma unroll
     for (int i = 0; i < BC_NC; ++i) vc[i] = sm.vs[q + 4 * i];
     const c128 vr = sm.vs[r];
-    // ---- w = D v (Hermitian D from its lower triangle), four independent accumulators
-    c128 wr;
+    // ---- the D phase (two-sided update of D_k) and the S phase (right update of S_{k+1}, next reflector) depend
+    //      only on (v, tau): their matrix-vector products run in one loop, their block-wide reductions share one
+    //      barrier, and the D update is issued next to the z products of the S phase (independent instruction streams)
+    const bool has_s = FULL || len2 > 0;
+    c128 wr, ur;
     {
-        c128 acc[4];
+        c128 accd[4], accs[4];
 #pragma unroll
-        for (int u = 0; u < 4; ++u) acc[u] = cmake(0.0, 0.0);
+        for (int u = 0; u < 4; ++u) accd[u] = accs[u] = cmake(0.0, 0.0);
 #pragma unroll
         for (int i = 0; i < BC_NC; ++i) {
             const int c = q + 4 * i;
             c128 e = cmake(0.0, 0.0);
             if (FULL || (r < len && c < len)) {
-                e = sm.D[c <= r ? r + c * BC_LD : c + r * BC_LD];
+                e = sm.D[c <= r ? r + c * BC_LD : c + r * BC_LD];      // Hermitian D from its lower triangle
                 if (c >= r) e.y = (c == r) ? 0.0 : -e.y;
             }
-            cfma(acc[i & 3], e, vc[i]);
+            cfma(accd[i & 3], e, vc[i]);
+            cfma(accs[i & 3], sreg[i], vc[i]);
         }
-        wr = cadd(cadd(acc[0], acc[1]), cadd(acc[2], acc[3]));
+        wr = cadd(cadd(accd[0], accd[1]), cadd(accd[2], accd[3]));
+        ur = cadd(cadd(accs[0], accs[1]), cadd(accs[2], accs[3]));
     }
     wr = cadd(wr, bc_shfl_xor(wr, 8));
+    ur = cadd(ur, bc_shfl_xor(ur, 8));
     wr = cadd(wr, bc_shfl_xor(wr, 16));
+    ur = cadd(ur, bc_shfl_xor(ur, 16));
+    // S <- S (I - tau v v^H) in registers:  S -= (tau u) v^H
+    {
+        const c128 tu = cmul(tau, ur);
+#pragma unroll
+        for (int i = 0; i < BC_NC; ++i) {
+            sreg[i].x -= tu.x * vc[i].x + tu.y * vc[i].y;
+            sreg[i].y -= tu.y * vc[i].x - tu.x * vc[i].y;
+        }
+    }
+    // partial sums of v^H (D v) and of the next reflector's norm (first column of S, held by the q = 0 lanes)
+    const c128 xs0 = cmake(__shfl_sync(0xffffffffu, sreg[0].x, rl), __shfl_sync(0xffffffffu, sreg[0].y, rl));
     {
         double pa = (q == 0) ? vr.x * wr.x + vr.y * wr.y : 0.0;   // Re(conj(v_r) w_r)
+        double pn = (q == 0 && r >= 1 && r < len2) ? cabs2(xs0) : 0.0;
         pa = bc_warp_sum(pa);
-        if (t.lane == 0) sm.red[t.warp] = pa;
+        pn = bc_warp_sum(pn);
+        if (t.lane == 0) { sm.red[t.warp] = pa; sm.red2[t.warp] = pn; }
         if (q == 0) sm.ws[r] = wr;
+        if (r == 0 && q == 0) sm.xs[0] = xs0;
     }
+    BC_STAMP(3);
     bc_sync_compute();
+    BC_STAMP(4);
+    // ---- next reflector (zlarfg scalars, redundantly in every thread)
+    c128 taun = cmake(0.0, 0.0);
+    double betan = 0.0;
+    c128 vnr = cmake(0.0, 0.0);
+    if (has_s) {
+        double xnorm2 = 0.0;
+#pragma unroll
+        for (int w = 0; w < BC_NW; ++w) xnorm2 += sm.red2[w];
+        c128 sc;
+        bc_reflector_scalars(sm.xs[0], xnorm2, taun, sc, betan);
+        if (r < len2) vnr = (r == 0) ? cmake(1.0, 0.0) : cmul(sc, xs0);
+    }
+    // ---- D <- D - v y^H - y v^H,  y = tau w - f v, f = 1/2 |tau|^2 (v^H w):
+    //      D[r,c] -= (conj(tau) v_r) conj(w_c) + (tau w_r - 2 f v_r) conj(v_c)   (lower triangle, straight to global)
     {
         double vhw = 0.0;
 #pragma unroll
         for (int w = 0; w < BC_NW; ++w) vhw += sm.red[w];
-        // y = tau w - f v, f = 1/2 |tau|^2 (v^H w);  D -= v y^H + y v^H = (conj(tau) v_r) conj(w_c) + (tau w_r - 2 f v_r) conj(v_c)
         const double f2 = (tau.x * tau.x + tau.y * tau.y) * vhw;
         const c128 pr = cmulc(tau, vr);                    // conj(tau) v_r
         const c128 twr = cmul(tau, wr);
@@ -222,32 +270,8 @@ __device__ __forceinline__ bool bc_step(BcSmem& sm, const BcStepCtx& t, int r0, 
             }
         }
     }
-    if (!FULL && len2 <= 0) return false;
-    // ---- S <- S (I - tau v v^H):  u = S v,  S -= (tau u) v^H   (all in registers)
-    {
-        c128 acc[4];
-#pragma unroll
-        for (int u = 0; u < 4; ++u) acc[u] = cmake(0.0, 0.0);
-#pragma unroll
-        for (int i = 0; i < BC_NC; ++i) cfma(acc[i & 3], sreg[i], vc[i]);
-        c128 ur = cadd(cadd(acc[0], acc[1]), cadd(acc[2], acc[3]));
-        ur = cadd(ur, bc_shfl_xor(ur, 8));
-        ur = cadd(ur, bc_shfl_xor(ur, 16));
-        const c128 tu = cmul(tau, ur);
-#pragma unroll
-        for (int i = 0; i < BC_NC; ++i) {
-            sreg[i].x -= tu.x * vc[i].x + tu.y * vc[i].y;
-            sreg[i].y -= tu.y * vc[i].x - tu.x * vc[i].y;
-        }
-    }
-    // ---- next reflector from the first column of S (held by the q = 0 lanes in sreg[0])
-    c128 taun;
-    double betan;
-    c128 vnr;
-    {
-        const c128 x = cmake(__shfl_sync(0xffffffffu, sreg[0].x, rl), __shfl_sync(0xffffffffu, sreg[0].y, rl));
-        vnr = bc_make_reflector(x, t, len2, sm.red2, &sm.xs[0], taun, betan);
-    }
+    if (!has_s) return false;
+    BC_STAMP(5);
     // ---- z_c = vn^H S[:, c]: per-thread products, reduce-scatter over the 8 row lanes, then across warps
     {
         c128 zp[BC_NC];
@@ -269,6 +293,7 @@ __device__ __forceinline__ bool bc_step(BcSmem& sm, const BcStepCtx& t, int r0, 
         sm.zpart[t.warp * BC_B + q + 4 * (ibase + 0)] = zp[0];
         sm.zpart[t.warp * BC_B + q + 4 * (ibase + 1)] = zp[1];
     }
+    BC_STAMP(6);
     bc_sync_compute();
     if (t.tid < BC_B) {
         c128 z0 = cadd(sm.zpart[0 * BC_B + t.tid], sm.zpart[1 * BC_B + t.tid]);
@@ -278,6 +303,7 @@ __device__ __forceinline__ bool bc_step(BcSmem& sm, const BcStepCtx& t, int r0, 
         sm.zs[t.tid] = cmulc(taun, cadd(cadd(z0, z1), cadd(z2, z3)));        // conj(tau') z_c
     }
     bc_sync_compute();
+    BC_STAMP(7);
     // ---- S[:, c] -= vn (conj(tau') z_c) for c >= 1; S[:, 0] = beta' e_1; store S and the reflector
     {
         c128* sp = band + (BC_B + r - q) + (int64_t)(r0 + q) * ldab;
@@ -300,6 +326,7 @@ __device__ __forceinline__ bool bc_step(BcSmem& sm, const BcStepCtx& t, int r0, 
     }
     if (t.tid == 0) t.tau2j[k + 1] = taun;
     tau = taun;
+    BC_STAMP(8);
     return true;
 }
 
@@ -367,6 +394,7 @@ __global__ void __launch_bounds__(BC_NT + 32, 1) bulge_chase_kernel(const BcArgs
             if (!more) break;
             if (tid == 0) bc_poll(a.progress, j - 1, k + 3);
             bc_sync_compute();
+            BC_STAMP(9);
         }
     }
 }
@@ -428,3 +456,16 @@ int phase_band_to_tridiag(eigh_handle_s* h, c128* band, int64_t ldab, double* d,
 }
 
 }  // namespace eigh
+
+#ifdef BC_PROFILE
+// developer-only build (-DBC_PROFILE): cycles accumulated between the stamps of bc_step, CTA-thread 0 of every block
+extern "C" int eigh_debug_bc_profile(unsigned long long out[16], int reset) {
+    cudaDeviceSynchronize();
+    cudaMemcpyFromSymbol(out, eigh::g_bc_prof, 16 * sizeof(unsigned long long));
+    if (reset) {
+        unsigned long long z[16] = {0};
+        cudaMemcpyToSymbol(eigh::g_bc_prof, z, sizeof(z));
+    }
+    return 0;
+}
+#endif
