@@ -396,7 +396,7 @@ def main():
                    "l2": "inputs larger than L2 (matrix %.1f GB)" % (mat_bytes / 1e9),
                    "input_regeneration": "device copy outside the timed brackets"},
         "clocks": clocks, "e2e": e2e, "gpu_launches": launches, "phases": phase_report, "roofline": roofline,
-        "cpu_baseline": cpu, "validity": valid,
+        "cpu_baseline": cpu, "validity": valid, "epilogue": epilogue,
         "total_tflops": (cw["p1_flops"] + cw["p2_flops"] + cw["p4a_flops"] + cw["p4b_flops"]) / ms_per_step / 1e9,
     }
     print(json.dumps(line))

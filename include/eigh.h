@@ -131,6 +131,27 @@ int eigh_backtransform_full(eigh_handle_t h, const void* A_dev, int64_t lda, voi
                             int64_t ldz, void* stream);
 
 /* ---------------------------------------------------------------------------------------
+ * SCF epilogue: the local densities the paper's self-consistent loop forms from the
+ * eigenpairs (Eq. 16a, 16d; Fermi factors Eq. 17):
+ *     n(r)  = 2 sum_{0 < E_n < E_c} ( |v_n(r)|^2 f_T(-E_n) + |u_n(r)|^2 f_T(E_n) )
+ *     nu(r) =   sum_{0 < E_n < E_c} u_n(r) conj(v_n(r)) ( f_T(-E_n) - f_T(E_n) ),   f_T(E) = 1 / (1 + exp(E / T)),
+ * with phi_n = [u_n, v_n]^T = column n of Z: rows [0, M) hold u_n(r), rows [M, 2M) hold v_n(r), M = N/2 (N even),
+ * lattice spacing 1.  One streaming pass over the active columns of Z (HBM-bound), summation order fixed
+ * (bit-reproducible).
+ *   E_dev  : ncols doubles, E_dev[j] = energy of column j of Z (any order; eigh_solve's W_dev qualifies).
+ *   Z_dev  : N x ncols c128, ldz >= N (read only).  0 <= ncols <= N.
+ *   T      : temperature >= 0; T = 0 is the step function.   Ec: cutoff (> 0; INFINITY = none).
+ *   branch : +1 = Eq. 16 as written, on the columns with 0 < E < Ec;
+ *            -1 = use the columns with -Ec < E < 0 in place of their particle-hole partners [-conj(v), conj(u)]
+ *                 of energy -E (valid for H = [[h, D], [D^*, -h^*]] with diagonal D): the lowest N/2 eigenpairs
+ *                 of H then give the same densities as the positive branch.
+ *   n_dev  : M doubles (out).   nu_dev : M c128 (out).
+ * Uses the handle's workspace (eigh_set_workspace must have been called); enqueues 3 kernels on `stream`,
+ * does not synchronise.  Returns -k for a bad k-th argument, -1 if N is odd. */
+int eigh_densities(eigh_handle_t h, const double* E_dev, const void* Z_dev, int64_t ldz, int64_t ncols,
+                   double T, double Ec, int branch, double* n_dev, void* nu_dev, void* stream);
+
+/* ---------------------------------------------------------------------------------------
  * Kernel-level entry points (unit tests and microbenchmarks of the building blocks).
  * ------------------------------------------------------------------------------------- */
 

@@ -35,6 +35,7 @@ SIGNATURES = {
     "eigh_tridiag_dc": (_int, [_vp, _vp, _vp, _vp, _vp, _i64, _vp]),
     "eigh_backtransform_band": (_int, [_vp, _vp, _i64, _vp, _i64, _vp]),
     "eigh_backtransform_full": (_int, [_vp, _vp, _i64, _vp, _i64, _vp]),
+    "eigh_densities": (_int, [_vp, _vp, _vp, _i64, _i64, _dbl, _dbl, _int, _vp, _vp, _vp]),
     "eigh_k_zgemm": (_int, [_vp, ctypes.c_char, ctypes.c_char, _i64, _i64, _i64, _dbl, _vp, _i64, _vp, _i64,
                             _i64, _vp, _i64, _vp, _i64, _dbl, _vp, _i64, _int, _int, _vp]),
     "eigh_k_zhemm_lower": (_int, [_vp, _i64, _i64, _vp, _i64, _vp, _i64, _vp, _i64, _int, _vp]),
@@ -143,6 +144,27 @@ class Eigh:
                                       _ptr(At_dev), _ptr(W_dev), _ptr(Zt_dev), _stream())
         self._check(rc, "eigh_solve_host")
         return W_host, Zt_host
+
+    # ------------------------------------------------------------------ SCF epilogue
+    def densities(self, E, Zt, T: float = 0.0, Ec: float = float("inf"), branch: int = 1, n=None, nu=None):
+        """eigh_densities (Eq. 16a, 16d, 17).  E: (ncols,) float64 energies of the rows of Zt; Zt: (ncols, N)
+        complex128 = Z column-major (as `solve` returns it; a row stride >= N is allowed).
+        Returns (n [N/2] float64, nu [N/2] complex128).  Enqueues only; no synchronisation."""
+        import torch
+        ncols = int(Zt.shape[0])
+        assert Zt.is_cuda and Zt.dtype == torch.complex128 and Zt.shape[1] == self.N
+        assert ncols == 0 or (Zt.stride(1) == 1 and (ncols == 1 or Zt.stride(0) >= self.N))
+        assert E.is_cuda and E.dtype == torch.float64 and E.is_contiguous() and E.numel() >= ncols
+        ldz = int(Zt.stride(0)) if ncols > 1 else self.N
+        M = self.N // 2
+        if n is None:
+            n = torch.empty(M, dtype=torch.float64, device=Zt.device)
+        if nu is None:
+            nu = torch.empty(M, dtype=torch.complex128, device=Zt.device)
+        rc = self.lib.eigh_densities(self.h, _ptr(E), _ptr(Zt), ldz, ncols, float(T), float(Ec), int(branch),
+                                     _ptr(n), _ptr(nu), _stream())
+        self._check(rc, "eigh_densities")
+        return n, nu
 
     def phase_times_ms(self):
         ms = (ctypes.c_double * 5)()

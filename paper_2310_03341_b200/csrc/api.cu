@@ -244,6 +244,24 @@ int eigh_backtransform_full(eigh_handle_t h, const void* A_dev, int64_t lda, voi
     return cuda_fail(h, phase_backtransform_full(h, (const c128*)A_dev, lda, (c128*)Z_dev, ldz, (cudaStream_t)stream), "backtransform_full");
 }
 
+int eigh_densities(eigh_handle_t h, const double* E_dev, const void* Z_dev, int64_t ldz, int64_t ncols, double T,
+                   double Ec, int branch, double* n_dev, void* nu_dev, void* stream) {
+    int rc = ensure_ready(h);
+    if (rc) return rc;
+    if (h->N & 1) return set_err(h, -1, "eigh_densities: N = %lld is odd (phi = [u, v] needs N = 2M)", (long long)h->N);
+    if (!E_dev && ncols > 0) return -2;
+    if (!Z_dev && ncols > 0) return -3;
+    if (ldz < h->N) return -4;
+    if (ncols < 0 || ncols > h->N) return -5;
+    if (!(T >= 0.0)) return -6;
+    if (Ec != Ec) return -7;
+    if (branch != 1 && branch != -1) return -8;
+    if (!n_dev) return -9;
+    if (!nu_dev) return -10;
+    return cuda_fail(h, launch_densities(h, E_dev, (const c128*)Z_dev, ldz, ncols, T, Ec, branch, n_dev, (c128*)nu_dev,
+                                         (cudaStream_t)stream), "densities");
+}
+
 int eigh_solve(eigh_handle_t h, void* A_dev, int64_t lda, double* W_dev, void* Z_dev, void* stream) {
     int rc = ensure_ready(h);
     if (rc) return rc;

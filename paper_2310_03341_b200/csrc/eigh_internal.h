@@ -97,6 +97,8 @@ int phase_backtransform_band(eigh_handle_s* h, const double* Q, int64_t ldq, c12
                              cudaStream_t s);
 int phase_backtransform_full(eigh_handle_s* h, const c128* A, int64_t lda, c128* Z, int64_t ldz,
                              cudaStream_t s);
-
+// SCF epilogue (densities.cu): n(r), nu(r) of Eq. 16a / 16d from the columns of Z
+int launch_densities(eigh_handle_s* h, const double* E, const c128* Z, int64_t ldz, int64_t ncols, double T, double Ec,
+                     int branch, double* n_out, c128* nu_out, cudaStream_t s);
 
 }  // namespace eigh

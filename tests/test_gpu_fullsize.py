@@ -138,6 +138,49 @@ def test_config3_positive_branch_nev_half():
     assert orth <= 1e-12 * N, orth
 
 
+def test_config3_densities_from_the_lowest_half():
+    """SCF epilogue at the size bench.py times (Eq. 16a, 16d, 17): nev = N/2 LOWEST pairs of H
+    (the negative branch) and eigh_densities with branch = -1.  The oracle recomputes n(r), nu(r) one point at a
+    time on 48 sampled grid points from the mapped states [-conj(v), conj(u)]; properties that hold at any size
+    cover every r: completeness n(r) -> 1, nu(r) -> 0 as T -> infinity, and the particle number."""
+    from oracle import densities as od
+    from paper_2310_03341_b200 import binding
+    w = wl.make_config(3)
+    N = w.N
+    M, nev = N // 2, N // 2
+    dev = torch.device("cuda")
+    At = torch.empty((N, N), dtype=torch.complex128, device=dev)
+    w.dense_torch(dev, out=At)
+    eng = binding.Eigh(N, nev)
+    W, Zt = eng.solve(At)
+    del At
+    assert float(W[nev - 1].item()) < 0.0 < float(W[nev].item())
+    E = W[:nev].contiguous()
+    pts = np.unique(np.linspace(0, M - 1, 48).astype(int))
+    rows = torch.from_numpy(np.concatenate([pts, M + pts])).to(dev)
+    Zs = Zt[:, rows].t().cpu().numpy()                   # (2 P) x nev: u rows then v rows of the sampled points
+    En = E.cpu().numpy()
+    for T, Ec in ((0.0, np.inf), (0.1, 8.0)):
+        n, nu = eng.densities(E, Zt, T=T, Ec=Ec, branch=-1)
+        torch.cuda.synchronize()
+        n, nu = n.cpu().numpy(), nu.cpu().numpy()
+        n_o, nu_o = od.densities(*od.particle_hole_map(En, Zs), T=T, Ec=Ec)
+        S = (np.abs(Zs) ** 2).sum(axis=1)
+        tol = 4.0 * nev * np.finfo(np.float64).eps * (S[:pts.size] + S[pts.size:])
+        assert np.all(np.abs(n[pts] - n_o) <= tol), np.abs(n[pts] - n_o).max()
+        assert np.all(np.abs(nu[pts] - nu_o) <= tol), np.abs(nu[pts] - nu_o).max()
+        assert np.all(n >= 0.0) and np.all(n <= 2.0 + 1e-9)
+        if T == 0.0:
+            # N_particles = sum_r n(r) = 2 sum_n ||v_n||^2 of the positive states = 2 sum ||u'||^2 of the mapped ones
+            unorm = float((Zt[:, :M].real ** 2 + Zt[:, :M].imag ** 2).sum().item())
+            assert abs(n.sum() - 2.0 * unorm) <= 1e-9 * n.sum()
+    n, nu = eng.densities(E, Zt, T=1e12, branch=-1)
+    torch.cuda.synchronize()
+    assert float((n - 1.0).abs().max().item()) <= 1e-9
+    assert float(nu.abs().max().item()) <= 1e-9
+    eng.close()
+
+
 @pytest.mark.skipif(os.environ.get("EIGH_TEST_C4", "0") != "1", reason="N = 49152 needs ~150 GB and minutes: set EIGH_TEST_C4=1")
 def test_config4_target_size_sampled():
     w, Hl, W, Zt, hn, tr, phases = _solve_config(4)
