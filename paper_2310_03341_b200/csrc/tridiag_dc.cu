@@ -516,9 +516,25 @@ __global__ void __launch_bounds__(256) dc_build_u_kernel(const MergeDesc* __rest
 }
 
 // ------------------------------------------------------------------ S3.5 merge GEMM descriptors, deflated columns
+// Last merge with nev < N: only the secular roots among the lowest nev values of the merged spectrum need their
+// eigenvector.  The roots are ascending in j, so those are a prefix j < kn; root j is wanted when fewer than nev
+// values lie below it: j roots plus the deflated values < lam_j (ties counted in favour of keeping the root).
+__global__ void __launch_bounds__(256) dc_wanted_kernel(const MergeDesc* __restrict__ desc, const int* __restrict__ kcount,
+                                                        const int* __restrict__ df_idx, const double* __restrict__ dcur,
+                                                        const double* __restrict__ lam, int nev, int* __restrict__ kn) {
+    const MergeDesc m = desc[0];
+    const int n = m.e - m.s, k = kcount[0];
+    const int j = blockIdx.x * blockDim.x + threadIdx.x;
+    if (j >= k) return;
+    const double lj = lam[m.s + j];
+    int below = j;
+    for (int t = 0; t < n - k && below < nev; ++t) below += (dcur[m.s + df_idx[m.s + t]] < lj) ? 1 : 0;
+    if (below < nev) atomicMax(kn, j + 1);
+}
+
 __global__ void dc_gemm_desc_kernel(const MergeDesc* __restrict__ desc, const int* __restrict__ kcount,
                                     const int* __restrict__ k1c, const int* __restrict__ k2c, int nmerge, int64_t ldq,
-                                    DgemmDesc* __restrict__ g) {
+                                    DgemmDesc* __restrict__ g, const int* __restrict__ kn) {
     const int mi = blockIdx.x * blockDim.x + threadIdx.x;
     if (mi >= nmerge) return;
     const MergeDesc m = desc[mi];
@@ -530,7 +546,7 @@ __global__ void dc_gemm_desc_kernel(const MergeDesc* __restrict__ desc, const in
     d.offA = d.offB = d.offC = m.s + (int64_t)m.s * ldq;
     d.offIdx = m.s;
     d.M = m.mid - m.s;
-    d.N = k;
+    d.N = kn ? min(k, *kn) : k;          // columns of U that are wanted (all of them unless this is the last merge, nev < N)
     d.K = k1 + k2;
     d.pad = 0;
     g[2 * mi] = d;
@@ -649,7 +665,14 @@ int phase_tridiag_dc(eigh_handle_s* h, const double* d, const double* e, double*
         dc_secular_kernel<<<dim3(gx128, cnt), 128, 0, st>>>(dd, B.kcount, B.dk, B.zk, B.rho, B.zsum, B.org, B.mu, B.lam, B.fail);
         dc_zhat_kernel<<<dim3(gx128, cnt), 128, 0, st>>>(dd, B.kcount, B.dk, B.zk, B.org, B.mu, B.zhat);
         dc_build_u_kernel<<<dim3(maxn, cnt), 256, 0, st>>>(dd, B.kcount, B.dk, B.org, B.mu, B.zhat, B.upos, B.U, ldq);
-        dc_gemm_desc_kernel<<<(unsigned)ceil_div(cnt, 128), 128, 0, st>>>(dd, B.kcount, B.k1c, B.k2c, cnt, ldq, B.gdesc);
+        const int* kn = nullptr;
+        if (nev < N && lv + 1 == level_cnt.size() && cnt == 1) {
+            EIGH_CUDA_OK(cudaMemsetAsync(B.fail + 16, 0, sizeof(int), st));
+            dc_wanted_kernel<<<gx256, 256, 0, st>>>(dd, B.kcount, B.df_idx, dcur, B.lam, nev, B.fail + 16);
+            ++h->launches;
+            kn = B.fail + 16;          // second counter in the 256-byte block of `fail`
+        }
+        dc_gemm_desc_kernel<<<(unsigned)ceil_div(cnt, 128), 128, 0, st>>>(dd, B.kcount, B.k1c, B.k2c, cnt, ldq, B.gdesc, kn);
         h->launches += 9;
         DgemmArgs ga;
         memset(&ga, 0, sizeof(ga));

@@ -183,3 +183,31 @@ def test_dc_random_and_subset(N, seed):
     assert Q2.shape == (N, nev)
     T = np.diag(d) + np.diag(e, 1) + np.diag(e, -1)
     assert np.linalg.norm(T @ Q2 - Q2 * W[None, :nev]) <= 1e-13 * np.linalg.norm(T)
+
+
+@pytest.mark.parametrize("nev_of", [lambda N: 1, lambda N: 7, lambda N: N // 2, lambda N: N - 1])
+def test_dc_subset_with_deflation_and_ties(nev_of):
+    """nev < N shortens the last merge to the wanted secular roots: the subset must equal the leading columns of
+    the full solve as a subspace, also when deflated values tie with or interleave the roots (Wilkinson pairs,
+    glued blocks, integer Clement spectrum, total deflation)."""
+    cases = []
+    m = 60
+    cases.append((np.abs(np.arange(-m, m + 1)).astype(float), np.ones(2 * m)))
+    d = np.tile(np.abs(np.arange(-10, 11)).astype(float), 8)
+    e = np.ones(len(d) - 1)
+    for c, glue in enumerate([1e-8, 1e-12, 0.0, 1e-6, 1e-14, 1e-10, 1e-15]):
+        e[21 * (c + 1) - 1] = glue
+    cases.append((d, e))
+    i = np.arange(1, 150)
+    cases.append((np.zeros(150), np.sqrt(i * (150 - i))))
+    cases.append((np.full(130, -1.5), np.zeros(129)))
+    for d, e in cases:
+        N = len(d)
+        nev = max(1, nev_of(N))
+        W, Q = run_dc(d, e)
+        W2, Q2 = run_dc(d, e, nev=nev)
+        assert np.array_equal(W2, W)
+        assert Q2.shape == (N, nev) and np.isfinite(Q2).all()
+        T = np.diag(d) + np.diag(e, 1) + np.diag(e, -1)
+        assert np.linalg.norm(T @ Q2 - Q2 * W[None, :nev]) <= 1e-13 * max(np.linalg.norm(T), 1.0) * np.sqrt(nev)
+        assert np.abs(Q2.T @ Q2 - np.eye(nev)).max() <= 1e-13 * max(1, N / 100)
