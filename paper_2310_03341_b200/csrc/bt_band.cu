@@ -217,6 +217,10 @@ __device__ __forceinline__ void dmma_p(double (&c)[2], double a, double b) {
         : "d"(a), "d"(b));
 }
 
+#ifndef BT_GAUSS2
+#define BT_GAUSS2 1
+#endif
+
 struct BtSweepArgs {
     c128* Z; int64_t ldz;
     int N, nev;
@@ -307,6 +311,37 @@ __device__ __forceinline__ void bt_apply_step(const c128* __restrict__ Vs, const
                 }
         }
         // ---- Z += Y V   (m = column of Z, n = row, k = reflector)
+#if BT_GAUSS2
+        // Three real products per complex multiply-add (Gauss): with y = ar + i ai and v = vx + i vy,
+        //   k1 = ar (vx + vy),  k2 = (ai - ar) vx,  k3 = (ar + ai) vy;   Re(y v) = k1 - k3,  Im(y v) = k1 + k2.
+        // k2 and k3 accumulate straight into zi and zr; k1 is summed over the block's 8 reflectors and added to both.
+#pragma unroll
+        for (int c = 0; c < NB; ++c) {
+            const int cb = cb0 + c;
+            double ar[2], df[2], ns[2];
+#pragma unroll
+            for (int h = 0; h < 2; ++h) {
+                ar[h] = yr[c][h];
+                df[h] = yi[c][h] - yr[c][h];
+                ns[h] = -(yr[c][h] + yi[c][h]);
+            }
+#pragma unroll
+            for (int p = cb; p <= cb + 8; ++p) {
+                double k1[2] = {0.0, 0.0};
+#pragma unroll
+                for (int h = 0; h < 2; ++h) {
+                    c128 v = cmake(0.0, 0.0);
+                    if ((p != cb || g >= 2 * t + h) && (p != cb + 8 || g < 2 * t + h))
+                        v = Vs[(8 * p + g) + (8 * cb + 2 * t + h) * BT_LDV];
+                    dmma_p(k1, ar[h], v.x + v.y);
+                    dmma_p(zi[p], df[h], v.x);
+                    dmma_p(zr[p], ns[h], v.y);
+                }
+                zr[p][0] += k1[0]; zr[p][1] += k1[1];
+                zi[p][0] += k1[0]; zi[p][1] += k1[1];
+            }
+        }
+#else
 #pragma unroll
         for (int c = 0; c < NB; ++c) {
             const int cb = cb0 + c;
@@ -325,6 +360,7 @@ __device__ __forceinline__ void bt_apply_step(const c128* __restrict__ Vs, const
                 }
             }
         }
+#endif
         if (tail) {
             // rows beyond the matrix are virtual: keep them zero (stale V rows may have touched them)
 #pragma unroll
