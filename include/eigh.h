@@ -151,6 +151,19 @@ int eigh_backtransform_full(eigh_handle_t h, const void* A_dev, int64_t lda, voi
 int eigh_densities(eigh_handle_t h, const double* E_dev, const void* Z_dev, int64_t ldz, int64_t ncols,
                    double T, double Ec, int branch, double* n_dev, void* nu_dev, void* stream);
 
+/* SCF prologue: assemble the dense BdG matrix of Eq. 5 / 7 from its fields,
+ *     H = sign * [[h, diag(Delta)], [diag(Delta)^*, -h^*]],   h = T + diag(V) - mu,
+ *     T = Kx (x) Iy (x) Iz + Ix (x) Ky (x) Iz + Ix (x) Iy (x) Kz   (Eq. 8: the kinetic term, one dense
+ *     real symmetric 1-D matrix per axis), grid point r = (ix ny + iy) nz + iz, matrix index s M + r, M = nx ny nz.
+ *   Kx_dev, Ky_dev, Kz_dev : nx x nx, ny x ny, nz x nz doubles, column-major, ld = their order.
+ *   V_dev : M doubles.   Delta_dev : M c128.   mu : chemical potential.   sign : +1 or -1 (the matrix of -H).
+ *   A_dev : N x N c128 (out), lda >= N = 2 M = the handle's N; ALL N^2 elements are written (both triangles).
+ * The diagonal is summed as ((Kx + Ky) + Kz + V) - mu.  One kernel on `stream` (HBM-write-bound, 16 N^2 bytes), no
+ * synchronisation, no workspace needed.  Returns -k for a bad k-th argument. */
+int eigh_assemble_bdg(eigh_handle_t h, int64_t nx, int64_t ny, int64_t nz, const double* Kx_dev,
+                      const double* Ky_dev, const double* Kz_dev, const double* V_dev, const void* Delta_dev,
+                      double mu, double sign, void* A_dev, int64_t lda, void* stream);
+
 /* ---------------------------------------------------------------------------------------
  * Kernel-level entry points (unit tests and microbenchmarks of the building blocks).
  * ------------------------------------------------------------------------------------- */

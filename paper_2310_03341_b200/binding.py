@@ -36,6 +36,7 @@ SIGNATURES = {
     "eigh_backtransform_band": (_int, [_vp, _vp, _i64, _vp, _i64, _vp]),
     "eigh_backtransform_full": (_int, [_vp, _vp, _i64, _vp, _i64, _vp]),
     "eigh_densities": (_int, [_vp, _vp, _vp, _i64, _i64, _dbl, _dbl, _int, _vp, _vp, _vp]),
+    "eigh_assemble_bdg": (_int, [_vp, _i64, _i64, _i64, _vp, _vp, _vp, _vp, _vp, _dbl, _dbl, _vp, _i64, _vp]),
     "eigh_k_zgemm": (_int, [_vp, ctypes.c_char, ctypes.c_char, _i64, _i64, _i64, _dbl, _vp, _i64, _vp, _i64,
                             _i64, _vp, _i64, _vp, _i64, _dbl, _vp, _i64, _int, _int, _vp]),
     "eigh_k_zhemm_lower": (_int, [_vp, _i64, _i64, _vp, _i64, _vp, _i64, _vp, _i64, _int, _vp]),
@@ -165,6 +166,25 @@ class Eigh:
                                      _ptr(n), _ptr(nu), _stream())
         self._check(rc, "eigh_densities")
         return n, nu
+
+    def assemble_bdg(self, shape, Kx, Ky, Kz, V, Delta, mu: float, At=None, sign: float = 1.0):
+        """eigh_assemble_bdg (Eq. 5/7/8).  Kx, Ky, Kz: (L, L) float64 symmetric 1-D kinetic matrices; V: (M,) float64;
+        Delta: (M,) complex128; all CUDA tensors.  Returns At, (N, N) complex128 = H column-major (ready for solve)."""
+        import torch
+        nx, ny, nz = (int(v) for v in shape)
+        for K, L in ((Kx, nx), (Ky, ny), (Kz, nz)):
+            assert K.is_cuda and K.dtype == torch.float64 and K.shape == (L, L) and K.is_contiguous()
+        M = nx * ny * nz
+        assert V.is_cuda and V.dtype == torch.float64 and V.numel() == M and V.is_contiguous()
+        assert Delta.is_cuda and Delta.dtype == torch.complex128 and Delta.numel() == M and Delta.is_contiguous()
+        if At is None:
+            At = torch.empty((self.N, self.N), dtype=torch.complex128, device=V.device)
+        assert At.is_cuda and At.dtype == torch.complex128 and At.shape == (self.N, self.N) and At.is_contiguous()
+        # symmetric K: row-major storage equals column-major storage
+        rc = self.lib.eigh_assemble_bdg(self.h, nx, ny, nz, _ptr(Kx), _ptr(Ky), _ptr(Kz), _ptr(V), _ptr(Delta),
+                                        float(mu), float(sign), _ptr(At), self.N, _stream())
+        self._check(rc, "eigh_assemble_bdg")
+        return At
 
     def phase_times_ms(self):
         ms = (ctypes.c_double * 5)()
