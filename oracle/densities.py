@@ -61,3 +61,39 @@ def particle_hole_map(E, Z):
     Zp[:M] = -np.conj(Z[M:])
     Zp[M:] = np.conj(Z[:M])
     return -E, Zp
+
+
+def gradient_densities(E, Z, shape, Dx, Dy, Dz, T=0.0, Ec=np.inf):
+    """Kinetic and current densities, Eq. (16b), (16c), written out state by state in FP64:
+
+        tau(r) = 2 sum_{0 < E_n < E_c} ( |grad v_n|^2 f_T(-E_n) + |grad u_n|^2 f_T(E_n) )                  (16b)
+        j(r)   = 2 sum_{0 < E_n < E_c} Im( v_n grad v_n^* f_T(-E_n) - u_n grad u_n^* f_T(E_n) )             (16c)
+
+    Reading: Eq. 16b prints the range "0 <= E_n <= E_r"; the range of (16a, c, d) is used for all four.
+    The gradient is applied along each axis through a dense real 1-D matrix (inputs Dx, Dy, Dz; the spectral
+    derivative of PAPER.md:113-115 in matrix form): (d_x u)(ix, iy, iz) = sum_i' Dx[ix, i'] u(i', iy, iz), etc.,
+    on the grid r = (ix ny + iy) nz + iz.  Returns tau (M,) and j (3, M)."""
+    E = np.asarray(E, dtype=np.float64)
+    Z = np.asarray(Z)
+    nx, ny, nz = shape
+    M = nx * ny * nz
+    D = [np.asarray(Dx, dtype=np.float64), np.asarray(Dy, dtype=np.float64), np.asarray(Dz, dtype=np.float64)]
+    tau = np.zeros(M, dtype=np.float64)
+    j = np.zeros((3, M), dtype=np.float64)
+
+    def grad(w):
+        w = w.reshape(nx, ny, nz)
+        return [np.einsum("ai,ijk->ajk", D[0], w).reshape(M),
+                np.einsum("bj,ijk->ibk", D[1], w).reshape(M),
+                np.einsum("ck,ijk->ijc", D[2], w).reshape(M)]
+
+    for c in range(Z.shape[1]):
+        if not (0.0 < E[c] < Ec):
+            continue
+        fm, fp = float(fermi(-E[c], T)), float(fermi(E[c], T))
+        u, v = Z[:M, c], Z[M:, c]
+        gu, gv = grad(u), grad(v)
+        for a in range(3):
+            tau += 2.0 * (np.abs(gv[a]) ** 2 * fm + np.abs(gu[a]) ** 2 * fp)
+            j[a] += 2.0 * np.imag(v * np.conj(gv[a]) * fm - u * np.conj(gu[a]) * fp)
+    return tau, j

@@ -165,7 +165,10 @@ int launch_densities(eigh_handle_s* h, const double* E, const c128* Z, int64_t l
     double* part = (double*)(base + off);
     const int64_t max_chunks = (int64_t)((h->plan.gemm_partial_bytes - off) / ((size_t)3 * M * sizeof(double)));
     const int64_t row_blocks = ceil_div(M, DP_THREADS);
-    int64_t nchunks = ceil_div((int64_t)h->num_sms * 8, row_blocks);
+    // one wave: as many chunks as keep every thread block co-resident (a partial second wave would double the time)
+    int occ = 0;
+    EIGH_CUDA_OK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, dens_partial_kernel, DP_THREADS, 0));
+    int64_t nchunks = std::max<int64_t>(1, (int64_t)h->num_sms * std::max(occ, 1) / row_blocks);
     nchunks = std::min(nchunks, ceil_div(std::max<int64_t>(ncols, 1), 2 * DP_UNROLL));
     nchunks = std::max<int64_t>(1, std::min(nchunks, std::min<int64_t>(max_chunks, 65535)));
     dens_weights_kernel<<<1, DW_THREADS, 0, s>>>(E, ncols, T, Ec, branch, act, nact);

@@ -44,6 +44,24 @@ def kinetic_1d(L: int) -> np.ndarray:
     return K / L
 
 
+def derivative_1d(L: int) -> np.ndarray:
+    """D_L[i,j] = (1/L) sum_n (i k_n) exp(i k_n (i-j)) = -(1/L) sum_n k_n sin(k_n (i-j)), k_n = 2 pi n / L.
+
+    Dense-matrix form of the spectral first derivative on the grid of PAPER.md:113-115; real antisymmetric circulant.
+    The unpaired Nyquist mode n = -L/2 (even L) has no real first derivative on the grid and is dropped, the usual
+    convention; D exp(i k x) = i k exp(i k x) for every other grid wave number.  An input of eigh_gradient_densities.
+    """
+    n = np.arange(-(L // 2), L - L // 2)
+    if L % 2 == 0:
+        n = n[1:]
+    k = 2.0 * np.pi * n / L
+    diff = np.arange(L)[:, None] - np.arange(L)[None, :]
+    D = np.zeros((L, L))
+    for kk in k:
+        D -= kk * np.sin(kk * diff)
+    return D / L
+
+
 def grid_coords(shape: Tuple[int, int, int]):
     Nx, Ny, Nz = shape
     x = np.arange(Nx) - (Nx - 1) / 2.0
