@@ -151,6 +151,23 @@ int eigh_backtransform_full(eigh_handle_t h, const void* A_dev, int64_t lda, voi
 int eigh_densities(eigh_handle_t h, const double* E_dev, const void* Z_dev, int64_t ldz, int64_t ncols,
                    double T, double Ec, int branch, double* n_dev, void* nu_dev, void* stream);
 
+/* Kinetic and current densities (Eq. 16b, 16c), same states, weights and `branch` rule as eigh_densities:
+ *     tau(r) = 2 sum ( |grad v_n|^2 f_T(-E_n) + |grad u_n|^2 f_T(E_n) )
+ *     j(r)   = 2 sum Im( v_n grad v_n^* f_T(-E_n) - u_n grad u_n^* f_T(E_n) )
+ * (Eq. 16b prints the range 0 <= E_n <= E_r; the range 0 < E_n < E_c of Eq. 16a/c/d is used.)  The gradient acts along
+ * each axis through a dense real 1-D matrix: (d_x u)(ix, iy, iz) = sum_i' Dx[ix, i'] u(i', iy, iz), grid point
+ * r = (ix ny + iy) nz + iz -- the matrix form of the spectral derivative of PAPER.md:113-115.
+ *   nx, ny, nz : grid extents, 1..64 each, 2 nx ny nz = N.
+ *   Dx_dev, Dy_dev, Dz_dev : nx x nx, ny x ny, nz x nz doubles, column-major (D[l + l2 * L] = D[l, l2]).
+ *   E_dev, Z_dev, ldz, ncols, T, Ec, branch : as for eigh_densities.
+ *   tau_dev : M doubles (out).   j_dev : 3 M doubles (out), j_dev[a * M + r] = component a (x, y, z) at r.
+ * One launch per axis (ALU-bound: 4 L FP64 FMAs per point, state and axis) + weights + ordered reduction; summation
+ * order fixed (bit-reproducible).  Uses the handle's workspace; enqueues on `stream`, does not synchronise. */
+int eigh_gradient_densities(eigh_handle_t h, int64_t nx, int64_t ny, int64_t nz, const double* Dx_dev,
+                            const double* Dy_dev, const double* Dz_dev, const double* E_dev, const void* Z_dev,
+                            int64_t ldz, int64_t ncols, double T, double Ec, int branch, double* tau_dev, double* j_dev,
+                            void* stream);
+
 /* SCF prologue: assemble the dense BdG matrix of Eq. 5 / 7 from its fields,
  *     H = sign * [[h, diag(Delta)], [diag(Delta)^*, -h^*]],   h = T + diag(V) - mu,
  *     T = Kx (x) Iy (x) Iz + Ix (x) Ky (x) Iz + Ix (x) Iy (x) Kz   (Eq. 8: the kinetic term, one dense

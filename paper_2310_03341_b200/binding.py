@@ -36,6 +36,8 @@ SIGNATURES = {
     "eigh_backtransform_band": (_int, [_vp, _vp, _i64, _vp, _i64, _vp]),
     "eigh_backtransform_full": (_int, [_vp, _vp, _i64, _vp, _i64, _vp]),
     "eigh_densities": (_int, [_vp, _vp, _vp, _i64, _i64, _dbl, _dbl, _int, _vp, _vp, _vp]),
+    "eigh_gradient_densities": (_int, [_vp, _i64, _i64, _i64, _vp, _vp, _vp, _vp, _vp, _i64, _i64, _dbl, _dbl, _int,
+                                       _vp, _vp, _vp]),
     "eigh_assemble_bdg": (_int, [_vp, _i64, _i64, _i64, _vp, _vp, _vp, _vp, _vp, _dbl, _dbl, _vp, _i64, _vp]),
     "eigh_k_zgemm": (_int, [_vp, ctypes.c_char, ctypes.c_char, _i64, _i64, _i64, _dbl, _vp, _i64, _vp, _i64,
                             _i64, _vp, _i64, _vp, _i64, _dbl, _vp, _i64, _int, _int, _vp]),
@@ -166,6 +168,27 @@ class Eigh:
                                      _ptr(n), _ptr(nu), _stream())
         self._check(rc, "eigh_densities")
         return n, nu
+
+    def gradient_densities(self, shape, Dx, Dy, Dz, E, Zt, T: float = 0.0, Ec: float = float("inf"), branch: int = 1):
+        """eigh_gradient_densities (Eq. 16b, 16c).  Dx, Dy, Dz: (L, L) float64 CUDA tensors holding D^T row-major, i.e.
+        D column-major (pass `D.t().contiguous()` of the logical matrix).  E, Zt as for `densities`.
+        Returns (tau [M] float64, j [3, M] float64)."""
+        import torch
+        nx, ny, nz = (int(v) for v in shape)
+        ncols = int(Zt.shape[0])
+        for D, L in ((Dx, nx), (Dy, ny), (Dz, nz)):
+            assert D.is_cuda and D.dtype == torch.float64 and D.shape == (L, L) and D.is_contiguous()
+        assert Zt.is_cuda and Zt.dtype == torch.complex128 and Zt.shape[1] == self.N
+        assert ncols == 0 or (Zt.stride(1) == 1 and (ncols == 1 or Zt.stride(0) >= self.N))
+        assert E.is_cuda and E.dtype == torch.float64 and E.is_contiguous() and E.numel() >= ncols
+        ldz = int(Zt.stride(0)) if ncols > 1 else self.N
+        M = self.N // 2
+        tau = torch.empty(M, dtype=torch.float64, device=Zt.device)
+        j = torch.empty((3, M), dtype=torch.float64, device=Zt.device)
+        rc = self.lib.eigh_gradient_densities(self.h, nx, ny, nz, _ptr(Dx), _ptr(Dy), _ptr(Dz), _ptr(E), _ptr(Zt), ldz,
+                                              ncols, float(T), float(Ec), int(branch), _ptr(tau), _ptr(j), _stream())
+        self._check(rc, "eigh_gradient_densities")
+        return tau, j
 
     def assemble_bdg(self, shape, Kx, Ky, Kz, V, Delta, mu: float, At=None, sign: float = 1.0):
         """eigh_assemble_bdg (Eq. 5/7/8).  Kx, Ky, Kz: (L, L) float64 symmetric 1-D kinetic matrices; V: (M,) float64;

@@ -262,6 +262,33 @@ int eigh_densities(eigh_handle_t h, const double* E_dev, const void* Z_dev, int6
                                          (cudaStream_t)stream), "densities");
 }
 
+int eigh_gradient_densities(eigh_handle_t h, int64_t nx, int64_t ny, int64_t nz, const double* Dx_dev,
+                            const double* Dy_dev, const double* Dz_dev, const double* E_dev, const void* Z_dev,
+                            int64_t ldz, int64_t ncols, double T, double Ec, int branch, double* tau_dev, double* j_dev,
+                            void* stream) {
+    int rc = ensure_ready(h);
+    if (rc) return rc;
+    if (nx < 1 || ny < 1 || nz < 1 || nx > 64 || ny > 64 || nz > 64)
+        return set_err(h, -2, "eigh_gradient_densities: grid extents must be 1..64 per axis");
+    if (2 * nx * ny * nz != h->N)
+        return set_err(h, -2, "eigh_gradient_densities: 2 nx ny nz = %lld != N = %lld", (long long)(2 * nx * ny * nz), (long long)h->N);
+    if (!Dx_dev) return -5;
+    if (!Dy_dev) return -6;
+    if (!Dz_dev) return -7;
+    if (!E_dev && ncols > 0) return -8;
+    if (!Z_dev && ncols > 0) return -9;
+    if (ldz < h->N) return -10;
+    if (ncols < 0 || ncols > h->N) return -11;
+    if (!(T >= 0.0)) return -12;
+    if (Ec != Ec) return -13;
+    if (branch != 1 && branch != -1) return -14;
+    if (!tau_dev) return -15;
+    if (!j_dev) return -16;
+    return cuda_fail(h, launch_gradient_densities(h, (int)nx, (int)ny, (int)nz, Dx_dev, Dy_dev, Dz_dev, E_dev, (const c128*)Z_dev,
+                                                  ldz, ncols, T, Ec, branch, tau_dev, j_dev, (cudaStream_t)stream),
+                     "gradient_densities");
+}
+
 int eigh_solve(eigh_handle_t h, void* A_dev, int64_t lda, double* W_dev, void* Z_dev, void* stream) {
     int rc = ensure_ready(h);
     if (rc) return rc;

@@ -150,6 +150,227 @@ __global__ void dens_reduce_kernel(const double* __restrict__ part, int nchunks,
     nu_out[r] = cmake(nr, ni);
 }
 
+// ------------------------------------------------------------------ Eq. 16b, 16c: kinetic and current densities
+//     tau(r) = 2 sum ( |grad v_n|^2 f_T(-E_n) + |grad u_n|^2 f_T(E_n) )
+//     j(r)   = 2 sum Im( v_n grad v_n^* f_T(-E_n) - u_n grad u_n^* f_T(E_n) )        (same states as Eq. 16a)
+// The gradient along an axis is a dense real L x L matrix applied to the lines of the grid along that axis.  With the
+// grid seen as (O, L, I) -- O outer, I inner points around the axis -- line lambda = o I + i holds the points
+// r = (o L + l) I + i, l = 0..L-1.  One launch per axis; a thread block owns a tile of 32 lines and loops over its
+// chunk of the active columns: the u and v tiles (L x 32 each) arrive by cp.async into a double buffer, every thread
+// (lane = line, warp = group of R = ceil(L/8) rows) forms (D u)(l) and (D v)(l) for its rows from shared memory and
+// adds the weighted |.|^2 and Im(w conj(D w)) terms to register partials.  In terms of the per-column weights of
+// Eq. 16a:  tau += wu |grad u|^2 + wv |grad v|^2,  j += wv Im(v grad v^*) - wu Im(u grad u^*)  (both branches).
+// ALU-bound: 4 L FP64 FMAs per grid point, state and axis against 32 bytes read per point, state and axis.
+constexpr int DG_THREADS = 256;
+constexpr int DG_C = 32;            // lines per tile
+constexpr int DG_PITCH = DG_C + 1;  // c128 elements per shared-memory row
+constexpr int DG_LMAX = 64;
+constexpr int DG_RMAX = DG_LMAX / 8;
+
+struct GradArgs {
+    const c128* Z; int64_t ldz; int64_t M;
+    int L; int64_t I; int64_t nlines;     // axis view (O, L, I); nlines = M / L
+    const double* D;                      // L x L, column-major: D[l + l2 * L] = D[l, l2]
+    const DensCol* act; const int* nact;
+    double* part_tau; double* part_j;     // this axis' partials: [chunk][M]
+};
+
+template <int R>
+__global__ void __launch_bounds__(DG_THREADS) dens_grad_kernel(const GradArgs p) {
+    extern __shared__ __align__(16) unsigned char dg_raw[];
+    const int L = p.L;
+    c128* buf = reinterpret_cast<c128*>(dg_raw);                  // [2 buffers][u, v][L][DG_PITCH]
+    double* Ds = reinterpret_cast<double*>(buf + (size_t)4 * L * DG_PITCH);   // Ds[l2 * LP + l], LP = 8 R
+    constexpr int LP = 8 * R;
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int64_t line0 = (int64_t)blockIdx.x * DG_C;
+    const int nchunks = gridDim.y, c = blockIdx.y;
+    const int nact = *p.nact;
+    const int len = (nact + nchunks - 1) / nchunks;
+    const int a0 = min(c * len, nact), a1 = min(a0 + len, nact);
+
+    for (int e = tid; e < L * LP; e += DG_THREADS) {
+        const int l2 = e / LP, l = e % LP;
+        Ds[e] = l < L ? p.D[l + (int64_t)l2 * L] : 0.0;
+    }
+    // this thread's elements of a tile: global offset (grid point) and shared-memory slot, fixed over the columns
+    constexpr int EMAX = DG_LMAX * DG_C / DG_THREADS;
+    int goff[EMAX], soff[EMAX];
+    const int nelem = L * DG_C;
+#pragma unroll
+    for (int k = 0; k < EMAX; ++k) {
+        const int e = tid + k * DG_THREADS;
+        goff[k] = -1;
+        soff[k] = 0;
+        if (e < nelem) {
+            int l, cc;
+            if (p.I == 1) { l = e % L; cc = e / L; }       // lines are contiguous in memory: run along l
+            else          { cc = e % DG_C; l = e / DG_C; } // neighbouring lines are contiguous: run along the lines
+            const int64_t line = line0 + cc;
+            soff[k] = l * DG_PITCH + cc;
+            if (line < p.nlines) {
+                const int64_t o = line / p.I, i = line % p.I;
+                goff[k] = (int)((o * L + l) * p.I + i);
+            }
+        }
+    }
+    auto issue = [&](int a, int b) {
+        const DensCol dc = p.act[a];
+        const c128* zu = p.Z + dc.col * p.ldz;
+        c128* ub = buf + (size_t)b * 2 * L * DG_PITCH;
+        c128* vb = ub + (size_t)L * DG_PITCH;
+#pragma unroll
+        for (int k = 0; k < EMAX; ++k) {
+            if (tid + k * DG_THREADS < nelem) {
+                const bool ok = goff[k] >= 0;
+                cp_async16(ub + soff[k], ok ? zu + goff[k] : zu, ok ? 16 : 0);
+                cp_async16(vb + soff[k], ok ? zu + p.M + goff[k] : zu, ok ? 16 : 0);
+            }
+        }
+    };
+    double tau[R], jj[R];
+#pragma unroll
+    for (int r = 0; r < R; ++r) tau[r] = jj[r] = 0.0;
+    if (a0 < a1) issue(a0, 0);
+    cp_async_commit();
+    for (int a = a0; a < a1; ++a) {
+        const int b = (a - a0) & 1;
+        if (a + 1 < a1) issue(a + 1, b ^ 1);
+        cp_async_commit();
+        cp_async_wait<1>();
+        __syncthreads();
+        const DensCol dc = p.act[a];
+        const c128* ub = buf + (size_t)b * 2 * L * DG_PITCH;
+        const c128* vb = ub + (size_t)L * DG_PITCH;
+        c128 gu[R], gv[R];
+#pragma unroll
+        for (int r = 0; r < R; ++r) gu[r] = gv[r] = cmake(0.0, 0.0);
+        for (int l2 = 0; l2 < L; ++l2) {
+            const c128 u = ub[l2 * DG_PITCH + lane], v = vb[l2 * DG_PITCH + lane];
+            const double* drow = Ds + l2 * LP + warp * R;
+#pragma unroll
+            for (int r = 0; r < R; ++r) {
+                const double d = drow[r];
+                gu[r].x = fma(d, u.x, gu[r].x); gu[r].y = fma(d, u.y, gu[r].y);
+                gv[r].x = fma(d, v.x, gv[r].x); gv[r].y = fma(d, v.y, gv[r].y);
+            }
+        }
+#pragma unroll
+        for (int r = 0; r < R; ++r) {
+            const int l = warp * R + r;
+            if (l < L) {
+                const c128 u = ub[l * DG_PITCH + lane], v = vb[l * DG_PITCH + lane];
+                tau[r] = fma(dc.wu, cabs2(gu[r]), tau[r]);
+                tau[r] = fma(dc.wv, cabs2(gv[r]), tau[r]);
+                jj[r] = fma(dc.wv, v.y * gv[r].x - v.x * gv[r].y, jj[r]);     // Im(v conj(g)) = v.y g.x - v.x g.y
+                jj[r] = fma(-dc.wu, u.y * gu[r].x - u.x * gu[r].y, jj[r]);
+            }
+        }
+        __syncthreads();      // the buffer is refilled two columns later, by the issue of the next iteration
+    }
+    cp_async_wait<0>();
+    const int64_t line = line0 + lane;
+    if (line < p.nlines) {
+        const int64_t o = line / p.I, i = line % p.I;
+#pragma unroll
+        for (int r = 0; r < R; ++r) {
+            const int l = warp * R + r;
+            if (l < L) {
+                const int64_t pt = (o * L + l) * p.I + i;
+                p.part_tau[(int64_t)c * p.M + pt] = tau[r];
+                p.part_j[(int64_t)c * p.M + pt] = jj[r];
+            }
+        }
+    }
+}
+
+// tau = sum over axes and chunks; j_a = sum over the chunks of axis a.  Partials: [axis][tau | j][chunk][M].
+__global__ void dens_grad_reduce_kernel(const double* __restrict__ part, int nchunks, int64_t M, double* __restrict__ tau,
+                                        double* __restrict__ j) {
+    const int64_t r = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (r >= M) return;
+    double t = 0.0;
+    for (int a = 0; a < 3; ++a) {
+        const double* pt = part + ((int64_t)(2 * a) * nchunks) * M;
+        const double* pj = part + ((int64_t)(2 * a + 1) * nchunks) * M;
+        double ja = 0.0;
+        for (int c = 0; c < nchunks; ++c) {
+            t += pt[(int64_t)c * M + r];
+            ja += pj[(int64_t)c * M + r];
+        }
+        j[(int64_t)a * M + r] = ja;
+    }
+    tau[r] = t;
+}
+
+template <int R>
+static int grad_axis(const GradArgs& a, int64_t ntiles, int nchunks, cudaStream_t s, int* occ) {
+    const size_t smem = (size_t)4 * a.L * DG_PITCH * sizeof(c128) + (size_t)a.L * 8 * R * sizeof(double);
+    EIGH_CUDA_OK(cudaFuncSetAttribute(dens_grad_kernel<R>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    if (occ) {       // query only: thread blocks of this axis' kernel that fit one SM
+        EIGH_CUDA_OK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(occ, dens_grad_kernel<R>, DG_THREADS, smem));
+        return 0;
+    }
+    dens_grad_kernel<R><<<dim3((unsigned)ntiles, (unsigned)nchunks), DG_THREADS, smem, s>>>(a);
+    return 0;
+}
+
+static int grad_axis_dispatch(const GradArgs& g, int64_t ntiles, int nchunks, cudaStream_t s, int* occ) {
+    switch ((int)ceil_div(g.L, 8)) {
+        case 1: return grad_axis<1>(g, ntiles, nchunks, s, occ);
+        case 2: return grad_axis<2>(g, ntiles, nchunks, s, occ);
+        case 3: return grad_axis<3>(g, ntiles, nchunks, s, occ);
+        case 4: return grad_axis<4>(g, ntiles, nchunks, s, occ);
+        case 5: return grad_axis<5>(g, ntiles, nchunks, s, occ);
+        case 6: return grad_axis<6>(g, ntiles, nchunks, s, occ);
+        case 7: return grad_axis<7>(g, ntiles, nchunks, s, occ);
+        default: return grad_axis<8>(g, ntiles, nchunks, s, occ);
+    }
+}
+
+int launch_gradient_densities(eigh_handle_s* h, int nx, int ny, int nz, const double* Dx, const double* Dy,
+                              const double* Dz, const double* E, const c128* Z, int64_t ldz, int64_t ncols, double T,
+                              double Ec, int branch, double* tau, double* j, cudaStream_t s) {
+    const int64_t M = h->N / 2;
+    char* base = ws_ptr<char>(h, h->plan.gemm_partial);
+    size_t off = 0;
+    DensCol* act = (DensCol*)(base + off);
+    off += (size_t)round_up(ncols * (int64_t)sizeof(DensCol) + 8, 256);
+    int* nact = (int*)(base + off) - 2;
+    if (off + (size_t)6 * M * sizeof(double) > h->plan.gemm_partial_bytes)
+        return set_err(h, -10, "eigh_gradient_densities: %lld columns do not fit the workspace", (long long)ncols);
+    double* part = (double*)(base + off);
+    const int64_t max_chunks = (int64_t)((h->plan.gemm_partial_bytes - off) / ((size_t)6 * M * sizeof(double)));
+    const int Ls[3] = {nx, ny, nz};
+    const int64_t Is[3] = {(int64_t)ny * nz, (int64_t)nz, 1};
+    const double* Ds[3] = {Dx, Dy, Dz};
+    GradArgs g[3];
+    int64_t ntiles[3];
+    // chunks of the active columns: as many as keep every thread block of every axis co-resident (one wave)
+    int64_t nchunks = std::min<int64_t>(std::min<int64_t>(max_chunks, 65535), ceil_div(std::max<int64_t>(ncols, 1), 8));
+    for (int a = 0; a < 3; ++a) {
+        g[a].Z = Z; g[a].ldz = ldz; g[a].M = M;
+        g[a].L = Ls[a]; g[a].I = Is[a]; g[a].nlines = M / Ls[a];
+        g[a].D = Ds[a]; g[a].act = act; g[a].nact = nact;
+        ntiles[a] = ceil_div(g[a].nlines, DG_C);
+        int occ = 0;
+        const int rc = grad_axis_dispatch(g[a], ntiles[a], 1, s, &occ);
+        if (rc) return rc;
+        nchunks = std::min<int64_t>(nchunks, (int64_t)h->num_sms * std::max(occ, 1) / ntiles[a]);
+    }
+    nchunks = std::max<int64_t>(1, nchunks);
+    dens_weights_kernel<<<1, DW_THREADS, 0, s>>>(E, ncols, T, Ec, branch, act, nact);
+    for (int a = 0; a < 3; ++a) {
+        g[a].part_tau = part + ((int64_t)(2 * a) * nchunks) * M;
+        g[a].part_j = part + ((int64_t)(2 * a + 1) * nchunks) * M;
+        const int rc = grad_axis_dispatch(g[a], ntiles[a], (int)nchunks, s, nullptr);
+        if (rc) return rc;
+    }
+    dens_grad_reduce_kernel<<<(unsigned)ceil_div(M, 256), 256, 0, s>>>(part, (int)nchunks, M, tau, j);
+    EIGH_CUDA_OK(cudaGetLastError());
+    return 0;
+}
+
 // Workspace use (the split-K partial region, idle outside the GEMMs): the active list (ncols entries + its length), then
 // the chunk partials.
 int launch_densities(eigh_handle_s* h, const double* E, const c128* Z, int64_t ldz, int64_t ncols, double T, double Ec,

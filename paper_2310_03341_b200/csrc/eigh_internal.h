@@ -33,7 +33,6 @@ struct WsPlan {
     size_t b4V, b4VT, b4Y, b4T, b4G;           // S4b merged-panel WY blocks: V, V T^H (N x kb), Y (kb x nev), T, G (kb x kb)
     size_t total;
 };
-
 }  // namespace eigh
 
 struct eigh_handle_s {
@@ -100,5 +99,8 @@ int phase_backtransform_full(eigh_handle_s* h, const c128* A, int64_t lda, c128*
 // SCF epilogue (densities.cu): n(r), nu(r) of Eq. 16a / 16d from the columns of Z
 int launch_densities(eigh_handle_s* h, const double* E, const c128* Z, int64_t ldz, int64_t ncols, double T, double Ec,
                      int branch, double* n_out, c128* nu_out, cudaStream_t s);
+int launch_gradient_densities(eigh_handle_s* h, int nx, int ny, int nz, const double* Dx, const double* Dy,
+                              const double* Dz, const double* E, const c128* Z, int64_t ldz, int64_t ncols, double T,
+                              double Ec, int branch, double* tau, double* j, cudaStream_t s);
 
 }  // namespace eigh

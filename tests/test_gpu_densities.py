@@ -146,3 +146,88 @@ def test_pipeline_vortex_vs_oracle_and_branches():
         eng.close()
         assert np.abs(n2.cpu().numpy() - n_o).max() <= 1e-10
         assert np.abs(nu2.cpu().numpy() - nu_o).max() <= 1e-10
+
+
+# ----------------------------------------------------------------------------- Eq. 16b, 16c: tau(r), j(r)
+def _gpu_gradient_densities(shape, Ds, E, Z, **kw):
+    from paper_2310_03341_b200 import binding
+    N = 2 * int(np.prod(shape))
+    ncols = Z.shape[1]
+    Zt = torch.from_numpy(np.ascontiguousarray(Z.T)).cuda() if ncols else torch.zeros((0, N), dtype=torch.complex128, device="cuda")
+    Ed = torch.from_numpy(np.ascontiguousarray(E)).cuda() if ncols else torch.zeros(1, dtype=torch.float64, device="cuda")
+    Dd = [torch.from_numpy(np.ascontiguousarray(D.T)).cuda() for D in Ds]      # column-major storage of D
+    eng = binding.Eigh(N)
+    tau, j = eng.gradient_densities(shape, Dd[0], Dd[1], Dd[2], Ed, Zt, **kw)
+    torch.cuda.synchronize()
+    eng.close()
+    return tau.cpu().numpy(), j.cpu().numpy()
+
+
+def _grad_tolerances(E, Z, shape, Ds, k):
+    """Both sides sum k states of products whose factors are L-term sums: |gpu - oracle| <= 8 (k + 2 L) eps S with
+    S >= sum_j |term_j|: for tau S = 2 max_r sum_j |grad u|^2 + |grad v|^2 (= 2 tau at f = 1/2, weights <= 2); for j the
+    Cauchy-Schwarz bound 2 sqrt(max_r sum |w|^2 * max_r sum |grad w|^2)."""
+    L = max(shape)
+    if Z.shape[1] == 0:
+        return 1e-300, 1e-300
+    Eall = np.ones(Z.shape[1])
+    t_inf, _ = od.gradient_densities(Eall, Z, shape, *Ds, T=1e12)      # = sum_j |grad u|^2 + |grad v|^2
+    n_inf, _ = od.densities(Eall, Z, T=1e12)                           # = sum_j |u|^2 + |v|^2
+    c = 8.0 * (k + 2 * L) * EPS
+    return c * 2.0 * t_inf.max(), c * 2.0 * np.sqrt(t_inf.max() * n_inf.max())
+
+
+@pytest.mark.parametrize("shape,ncols", [((1, 1, 2), 3), ((3, 5, 7), 40), ((8, 8, 8), 333), ((6, 10, 9), 1080), ((2, 33, 3), 17),
+                                         ((4, 4, 6), 0), ((9, 1, 40), 100)])
+@pytest.mark.parametrize("T,Ec", [(0.0, np.inf), (0.3, 1.1)])
+def test_gradient_densities_elementwise(shape, ncols, T, Ec):
+    """Distinct, non-antisymmetric random 1-D matrices (a transposed or swapped matrix shows); tiles with ragged ends
+    along every axis (lines not a multiple of 32), L from 1 to 40, empty input."""
+    M = int(np.prod(shape))
+    rng = np.random.default_rng(M + ncols)
+    Ds = [wl.derivative_1d(L) + 0.1 * rng.standard_normal((L, L)) for L in shape]
+    E, Z = _random_states(M, ncols, 31 * M + ncols)
+    tau, j = _gpu_gradient_densities(shape, Ds, E, Z, T=T, Ec=Ec)
+    tau_o, j_o = od.gradient_densities(E, Z, shape, *Ds, T=T, Ec=Ec)
+    tt, tj = _grad_tolerances(E, Z, shape, Ds, ncols)
+    assert np.abs(tau - tau_o).max() <= tt, (np.abs(tau - tau_o).max(), tt)
+    assert np.abs(j - j_o).max() <= tj, (np.abs(j - j_o).max(), tj)
+    if ncols == 0:
+        assert not tau.any() and not j.any()
+
+
+def test_gradient_densities_negative_branch():
+    shape, ncols = (5, 6, 7), 150
+    M = int(np.prod(shape))
+    Ds = [wl.derivative_1d(L) for L in shape]
+    E, Z = _random_states(M, ncols, 99)
+    tau, j = _gpu_gradient_densities(shape, Ds, E, Z, T=0.2, Ec=1.5, branch=-1)
+    tau_o, j_o = od.gradient_densities(*od.particle_hole_map(E, Z), shape, *Ds, T=0.2, Ec=1.5)
+    tt, tj = _grad_tolerances(E, Z, shape, Ds, ncols)
+    assert np.abs(tau - tau_o).max() <= tt and np.abs(j - j_o).max() <= tj
+
+
+def test_pipeline_moving_condensate_current():
+    """Delta = D0 exp(2 i q r) on a 5x5x7 grid, end to end on the GPU (assemble -> solve -> gradient densities) against
+    the oracle chain; the current is uniform, along q, and j_y = 0 (closed form pinned in test_oracle_densities.py)."""
+    from paper_2310_03341_b200 import binding
+    shape = (5, 5, 7)
+    nx, ny, nz = shape
+    M = nx * ny * nz
+    X, Y, Zc = np.meshgrid(np.arange(nx), np.arange(ny), np.arange(nz), indexing="ij")
+    Delta = 0.3 * np.exp(2j * (2 * np.pi / nx * X + 2 * 2 * np.pi / nz * Zc)).reshape(-1)
+    p = wl.BdGProblem("moving", shape, 0.9, np.zeros(M), Delta)
+    Ds = [wl.derivative_1d(L) for L in shape]
+    Wo, Zo = oracle.eigh(p.dense())
+    tau_o, j_o = od.gradient_densities(Wo, Zo, shape, *Ds, T=0.0)
+    dev = lambda a: torch.from_numpy(np.ascontiguousarray(a)).cuda()   # noqa: E731
+    eng = binding.Eigh(2 * M)
+    At = eng.assemble_bdg(shape, *[dev(wl.kinetic_1d(L)) for L in shape], dev(p.V), dev(p.Delta), p.mu)
+    W, Zt = eng.solve(At)
+    tau, j = eng.gradient_densities(shape, *[dev(D.T) for D in Ds], W, Zt, T=0.0)
+    torch.cuda.synchronize()
+    eng.close()
+    assert np.abs(tau.cpu().numpy() - tau_o).max() <= 1e-10
+    assert np.abs(j.cpu().numpy() - j_o).max() <= 1e-10
+    jn = j.cpu().numpy()
+    assert np.abs(jn[1]).max() <= 1e-10 and np.abs(jn[0]).min() > 1e-3 and np.abs(jn[0] - jn[0].mean()).max() <= 1e-10
