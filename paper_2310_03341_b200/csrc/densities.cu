@@ -156,16 +156,17 @@ __global__ void dens_reduce_kernel(const double* __restrict__ part, int nchunks,
 // The gradient along an axis is a dense real L x L matrix applied to the lines of the grid along that axis.  With the
 // grid seen as (O, L, I) -- O outer, I inner points around the axis -- line lambda = o I + i holds the points
 // r = (o L + l) I + i, l = 0..L-1.  One launch per axis; a thread block owns a tile of 32 lines and loops over its
-// chunk of the active columns: the u and v tiles (L x 32 each) arrive by cp.async into a double buffer, every thread
-// (lane = line, warp = group of R = ceil(L/8) rows) forms (D u)(l) and (D v)(l) for its rows from shared memory and
-// adds the weighted |.|^2 and Im(w conj(D w)) terms to register partials.  In terms of the per-column weights of
-// Eq. 16a:  tau += wu |grad u|^2 + wv |grad v|^2,  j += wv Im(v grad v^*) - wu Im(u grad u^*)  (both branches).
-// ALU-bound: 4 L FP64 FMAs per grid point, state and axis against 32 bytes read per point, state and axis.
+// chunk of the active columns: the u and v tiles (L x 32 each) arrive by cp.async into a double buffer, the products
+// (D u), (D v) of the tile run on the FP64 tensor cores (see the kernel), and each thread adds the weighted |.|^2 and
+// Im(w conj(D w)) terms of its grid points to register partials.  In terms of the per-column weights of Eq. 16a:
+//     tau += wu |grad u|^2 + wv |grad v|^2,     j += wv Im(v grad v^*) - wu Im(u grad u^*)        (both branches).
+// Bound by FP64 arithmetic: 4 L FMAs per grid point, state and axis against 32 bytes read per point, state and axis.
 constexpr int DG_THREADS = 256;
 constexpr int DG_C = 32;            // lines per tile
-constexpr int DG_PITCH = DG_C + 1;  // c128 elements per shared-memory row
+constexpr int DG_PITCH = DG_C + 2;  // c128 elements per shared-memory row: 544 B = 32 (mod 128), conflict-free B fragments
 constexpr int DG_LMAX = 64;
-constexpr int DG_RMAX = DG_LMAX / 8;
+// cp.async ring: tiles of 2 columns in flight while one is multiplied (1 column for L > 56, where 3 stages do not fit)
+__host__ __device__ constexpr int dg_stages(int MB) { return MB >= 8 ? 2 : 3; }
 
 struct GradArgs {
     const c128* Z; int64_t ldz; int64_t M;
@@ -175,26 +176,38 @@ struct GradArgs {
     double* part_tau; double* part_j;     // this axis' partials: [chunk][M]
 };
 
-template <int R>
-__global__ void __launch_bounds__(DG_THREADS) dens_grad_kernel(const GradArgs p) {
+// (D w)(l, line) for w = u, v as ONE real product on the FP64 tensor cores: G (LP x 128) = D (LP x LP) W (LP x 128),
+// the 128 real columns being (u | v) x 32 lines x (re, im); LP = 8 MB >= L, the padding rows of W and rows / columns
+// of D are zero.  Warp w owns lines 4w..4w+3 of both u and v: two 8-column blocks; in the accumulator layout of
+// mma.m8n8k4 (c0, c1 = columns 2t, 2t+1 of row g) every thread holds the complex values (D u), (D v) of the grid points
+// (l = 8 mb + g, line = 4w + t), mb = 0..MB-1, so the |.|^2 and Im(w conj(D w)) terms are formed in registers.
+// The A fragments (D) do not depend on the column: they are loaded once, into registers for MB <= 4 (L <= 32).
+template <int MB>
+__global__ void __launch_bounds__(DG_THREADS, MB <= 4 ? 2 : 1) dens_grad_kernel(const GradArgs p) {
     extern __shared__ __align__(16) unsigned char dg_raw[];
+    constexpr int LP = 8 * MB, KS = 2 * MB, DG_STAGES = dg_stages(MB);
+    constexpr bool A_IN_REGS = MB <= 4;
     const int L = p.L;
-    c128* buf = reinterpret_cast<c128*>(dg_raw);                  // [2 buffers][u, v][L][DG_PITCH]
-    double* Ds = reinterpret_cast<double*>(buf + (size_t)4 * L * DG_PITCH);   // Ds[l2 * LP + l], LP = 8 R
-    constexpr int LP = 8 * R;
+    c128* buf = reinterpret_cast<c128*>(dg_raw);                  // [DG_STAGES buffers][u, v][LP][DG_PITCH]
+    double* Ds = reinterpret_cast<double*>(buf + (size_t)2 * DG_STAGES * LP * DG_PITCH);   // Ds[l * (LP + 1) + l2]
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int g = lane >> 2, t = lane & 3;
     const int64_t line0 = (int64_t)blockIdx.x * DG_C;
     const int nchunks = gridDim.y, c = blockIdx.y;
     const int nact = *p.nact;
     const int len = (nact + nchunks - 1) / nchunks;
     const int a0 = min(c * len, nact), a1 = min(a0 + len, nact);
 
-    for (int e = tid; e < L * LP; e += DG_THREADS) {
-        const int l2 = e / LP, l = e % LP;
-        Ds[e] = l < L ? p.D[l + (int64_t)l2 * L] : 0.0;
+    for (int e = tid; e < LP * LP; e += DG_THREADS) {
+        const int l = e / LP, l2 = e % LP;
+        Ds[l * (LP + 1) + l2] = (l < L && l2 < L) ? p.D[l + (int64_t)l2 * L] : 0.0;
+    }
+    for (int e = tid; e < 2 * DG_STAGES * (LP - L) * DG_PITCH; e += DG_THREADS) {      // padding rows of all tiles stay zero
+        const int q = e / ((LP - L) * DG_PITCH), rem = e % ((LP - L) * DG_PITCH);
+        buf[(size_t)q * LP * DG_PITCH + (size_t)L * DG_PITCH + rem] = cmake(0.0, 0.0);
     }
     // this thread's elements of a tile: global offset (grid point) and shared-memory slot, fixed over the columns
-    constexpr int EMAX = DG_LMAX * DG_C / DG_THREADS;
+    constexpr int EMAX = LP * DG_C / DG_THREADS;       // = MB
     int goff[EMAX], soff[EMAX];
     const int nelem = L * DG_C;
 #pragma unroll
@@ -217,8 +230,8 @@ __global__ void __launch_bounds__(DG_THREADS) dens_grad_kernel(const GradArgs p)
     auto issue = [&](int a, int b) {
         const DensCol dc = p.act[a];
         const c128* zu = p.Z + dc.col * p.ldz;
-        c128* ub = buf + (size_t)b * 2 * L * DG_PITCH;
-        c128* vb = ub + (size_t)L * DG_PITCH;
+        c128* ub = buf + (size_t)b * 2 * LP * DG_PITCH;
+        c128* vb = ub + (size_t)LP * DG_PITCH;
 #pragma unroll
         for (int k = 0; k < EMAX; ++k) {
             if (tid + k * DG_THREADS < nelem) {
@@ -228,57 +241,70 @@ __global__ void __launch_bounds__(DG_THREADS) dens_grad_kernel(const GradArgs p)
             }
         }
     };
-    double tau[R], jj[R];
 #pragma unroll
-    for (int r = 0; r < R; ++r) tau[r] = jj[r] = 0.0;
-    if (a0 < a1) issue(a0, 0);
-    cp_async_commit();
-    for (int a = a0; a < a1; ++a) {
-        const int b = (a - a0) & 1;
-        if (a + 1 < a1) issue(a + 1, b ^ 1);
+    for (int st = 0; st < DG_STAGES - 1; ++st) {       // prefetch distance DG_STAGES - 1 columns
+        if (a0 + st < a1) issue(a0 + st, st);
         cp_async_commit();
-        cp_async_wait<1>();
-        __syncthreads();
+    }
+    __syncthreads();                                   // Ds is complete
+    double afr[A_IN_REGS ? MB : 1][A_IN_REGS ? KS : 1];
+    if constexpr (A_IN_REGS) {
+#pragma unroll
+        for (int mb = 0; mb < MB; ++mb)
+#pragma unroll
+            for (int ks = 0; ks < KS; ++ks) afr[mb][ks] = Ds[(8 * mb + g) * (LP + 1) + 4 * ks + t];
+    }
+    double tau[MB], jj[MB];
+#pragma unroll
+    for (int mb = 0; mb < MB; ++mb) tau[mb] = jj[mb] = 0.0;
+    const int myline = 4 * warp + t;                   // the line whose (re, im) this thread accumulates
+    for (int a = a0; a < a1; ++a) {
+        const int b = (a - a0) % DG_STAGES;
+        cp_async_wait<DG_STAGES - 2>();                // column a has landed (this thread's copies) ...
+        __syncthreads();                               // ... and everybody's; buffer (b - 1) is free again
+        if (a + DG_STAGES - 1 < a1) issue(a + DG_STAGES - 1, (b + DG_STAGES - 1) % DG_STAGES);
+        cp_async_commit();
         const DensCol dc = p.act[a];
-        const c128* ub = buf + (size_t)b * 2 * L * DG_PITCH;
-        const c128* vb = ub + (size_t)L * DG_PITCH;
-        c128 gu[R], gv[R];
+        const c128* ub = buf + (size_t)b * 2 * LP * DG_PITCH;
+        const c128* vb = ub + (size_t)LP * DG_PITCH;
+        // B fragment: row 4 ks + t, real column g of the warp's block = (line 4w + g/2, part g & 1)
+        const double* ubd = reinterpret_cast<const double*>(ub) + 2 * (4 * warp) + g;
+        const double* vbd = reinterpret_cast<const double*>(vb) + 2 * (4 * warp) + g;
+        double gu[MB][2], gv[MB][2];
 #pragma unroll
-        for (int r = 0; r < R; ++r) gu[r] = gv[r] = cmake(0.0, 0.0);
-        for (int l2 = 0; l2 < L; ++l2) {
-            const c128 u = ub[l2 * DG_PITCH + lane], v = vb[l2 * DG_PITCH + lane];
-            const double* drow = Ds + l2 * LP + warp * R;
+        for (int mb = 0; mb < MB; ++mb) gu[mb][0] = gu[mb][1] = gv[mb][0] = gv[mb][1] = 0.0;
 #pragma unroll
-            for (int r = 0; r < R; ++r) {
-                const double d = drow[r];
-                gu[r].x = fma(d, u.x, gu[r].x); gu[r].y = fma(d, u.y, gu[r].y);
-                gv[r].x = fma(d, v.x, gv[r].x); gv[r].y = fma(d, v.y, gv[r].y);
+        for (int ks = 0; ks < KS; ++ks) {
+            const double bu = ubd[(size_t)(4 * ks + t) * (2 * DG_PITCH)];
+            const double bv = vbd[(size_t)(4 * ks + t) * (2 * DG_PITCH)];
+#pragma unroll
+            for (int mb = 0; mb < MB; ++mb) {
+                const double av = A_IN_REGS ? afr[A_IN_REGS ? mb : 0][A_IN_REGS ? ks : 0] : Ds[(8 * mb + g) * (LP + 1) + 4 * ks + t];
+                dmma884p(gu[mb][0], gu[mb][1], av, bu);
+                dmma884p(gv[mb][0], gv[mb][1], av, bv);
             }
         }
 #pragma unroll
-        for (int r = 0; r < R; ++r) {
-            const int l = warp * R + r;
-            if (l < L) {
-                const c128 u = ub[l * DG_PITCH + lane], v = vb[l * DG_PITCH + lane];
-                tau[r] = fma(dc.wu, cabs2(gu[r]), tau[r]);
-                tau[r] = fma(dc.wv, cabs2(gv[r]), tau[r]);
-                jj[r] = fma(dc.wv, v.y * gv[r].x - v.x * gv[r].y, jj[r]);     // Im(v conj(g)) = v.y g.x - v.x g.y
-                jj[r] = fma(-dc.wu, u.y * gu[r].x - u.x * gu[r].y, jj[r]);
-            }
+        for (int mb = 0; mb < MB; ++mb) {
+            const int l = 8 * mb + g;
+            const c128 u = ub[l * DG_PITCH + myline], v = vb[l * DG_PITCH + myline];    // zero on the padding rows
+            tau[mb] = fma(dc.wu, gu[mb][0] * gu[mb][0] + gu[mb][1] * gu[mb][1], tau[mb]);
+            tau[mb] = fma(dc.wv, gv[mb][0] * gv[mb][0] + gv[mb][1] * gv[mb][1], tau[mb]);
+            jj[mb] = fma(dc.wv, v.y * gv[mb][0] - v.x * gv[mb][1], jj[mb]);     // Im(v conj(g)) = v.y g.x - v.x g.y
+            jj[mb] = fma(-dc.wu, u.y * gu[mb][0] - u.x * gu[mb][1], jj[mb]);
         }
-        __syncthreads();      // the buffer is refilled two columns later, by the issue of the next iteration
     }
     cp_async_wait<0>();
-    const int64_t line = line0 + lane;
+    const int64_t line = line0 + myline;
     if (line < p.nlines) {
         const int64_t o = line / p.I, i = line % p.I;
 #pragma unroll
-        for (int r = 0; r < R; ++r) {
-            const int l = warp * R + r;
+        for (int mb = 0; mb < MB; ++mb) {
+            const int l = 8 * mb + g;
             if (l < L) {
                 const int64_t pt = (o * L + l) * p.I + i;
-                p.part_tau[(int64_t)c * p.M + pt] = tau[r];
-                p.part_j[(int64_t)c * p.M + pt] = jj[r];
+                p.part_tau[(int64_t)c * p.M + pt] = tau[mb];
+                p.part_j[(int64_t)c * p.M + pt] = jj[mb];
             }
         }
     }
@@ -305,7 +331,8 @@ __global__ void dens_grad_reduce_kernel(const double* __restrict__ part, int nch
 
 template <int R>
 static int grad_axis(const GradArgs& a, int64_t ntiles, int nchunks, cudaStream_t s, int* occ) {
-    const size_t smem = (size_t)4 * a.L * DG_PITCH * sizeof(c128) + (size_t)a.L * 8 * R * sizeof(double);
+    constexpr int LP = 8 * R, DG_STAGES = dg_stages(R);
+    const size_t smem = (size_t)2 * DG_STAGES * LP * DG_PITCH * sizeof(c128) + (size_t)LP * (LP + 1) * sizeof(double);
     EIGH_CUDA_OK(cudaFuncSetAttribute(dens_grad_kernel<R>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     if (occ) {       // query only: thread blocks of this axis' kernel that fit one SM
         EIGH_CUDA_OK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(occ, dens_grad_kernel<R>, DG_THREADS, smem));
