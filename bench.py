@@ -326,8 +326,29 @@ def main():
                         "frac": (dbytes / dms / 1e6) / hbm if hbm and dms else None, "launches": 3,
                         "particle_number": float(n_f.sum().item()),
                         "note": "inputs (%.1f GB of active columns) larger than L2" % (16.0 * N * active / 1e9)}
-            # prologue: eigh_assemble_bdg writes all N^2 elements of H from (K, V, Delta): HBM-write-bound, 16 N^2 bytes
+            # Eq. 16b/16c: eigh_gradient_densities (three launches, one per axis; FP64 tensor cores + HBM: 4 L FMAs and 32
+            # bytes per grid point, state and axis -- at L = 24..32 the two rooflines nearly coincide, both are reported)
             pb = w.problem
+            Dd = [torch.from_numpy(np.ascontiguousarray(wl_mod.derivative_1d(L).T)).to(dev) for L in pb.shape]
+            solver.gradient_densities(pb.shape, Dd[0], Dd[1], Dd[2], W, Zt, T=0.0)
+            torch.cuda.synchronize()
+            ts = []
+            for _ in range(3):
+                ev0.record(stream)
+                solver.gradient_densities(pb.shape, Dd[0], Dd[1], Dd[2], W, Zt, T=0.0)
+                ev1.record(stream)
+                torch.cuda.synchronize()
+                ts.append(ev0.elapsed_time(ev1))
+            gms = sorted(ts)[len(ts) // 2]
+            gflops = 2.0 * 4.0 * sum(pb.shape) * (N // 2) * active          # 4 L FMAs per point, state and axis
+            gbytes = 3.0 * 16.0 * N * active
+            epilogue["gradient"] = {"op": "eigh_gradient_densities (Eq. 16b, 16c; T = 0)", "ms": gms, "launches": 5,
+                                    "algorithmic_flops": gflops, "algorithmic_bytes": gbytes, "bound": "tensor",
+                                    "achieved_tflops": gflops / gms / 1e9 if gms else None, "peak_tflops": FP64_NOMINAL_TFLOPS,
+                                    "frac": gflops / gms / 1e9 / FP64_NOMINAL_TFLOPS if gms else None,
+                                    "achieved_gbs": gbytes / gms / 1e6 if gms else None,
+                                    "hbm_frac": (gbytes / gms / 1e6) / hbm if hbm and gms else None}
+            # prologue: eigh_assemble_bdg writes all N^2 elements of H from (K, V, Delta): HBM-write-bound, 16 N^2 bytes
             Kd = [torch.from_numpy(wl_mod.kinetic_1d(L)).to(dev) for L in pb.shape]
             Vd = torch.from_numpy(pb.V).to(dev)
             Dd = torch.from_numpy(np.ascontiguousarray(pb.Delta)).to(dev)
