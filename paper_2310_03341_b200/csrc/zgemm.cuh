@@ -194,67 +194,81 @@ __global__ void __launch_bounds__(32 * WARPS_M * WARPS_N, MINB) zgemm_kernel(con
         return TA;
     };
 
-    auto load_stage = [&](int stage, int kb) {
-        c128* As = smem + (size_t)stage * Cfg::STAGE;
-        c128* Bs = As + Cfg::A_STAGE;
+    // Sequential tile loader.  The blocks kb_begin, kb_begin + 1, ... are requested in order, so every thread keeps, for
+    // its NA + NB elements of a stage, the global pointer, the shared-memory slot and the validity of its row / column, and
+    // only advances the pointers from block to block.  The state is rebuilt where the operands change: at the start, at
+    // the switch to the second (A2, B2) pair and, in HEMM mode, where the A tile turns from "as stored" to "mirrored".
+    constexpr int NA = BM * BK / NT, NB = BN * BK / NT;
+    const c128* pA[NA];
+    const c128* pB[NB];
+    int sA[NA], sB[NB], kA[NA], kB[NB];
+    bool vA[NA], vB[NB];
+    int64_t dA = 0, dB = 0;
+    int ld_kb = kb_begin, ld_switch = kb_begin, ld_krem = 0;
+    const c128* ld_safe = p.A1;
+    auto ld_setup = [&](int kb) {
         const bool second = kb >= nkb1;
         const c128* A = second ? p.A2 : p.A1;
         const c128* B = second ? p.B2 : p.B1;
         const int64_t lda = second ? p.lda2 : p.lda1, ldb = second ? p.ldb2 : p.ldb1;
         const int Kp = second ? p.K2 : p.K1;
         const int k0 = (second ? kb - nkb1 : kb) * BK;
-        if (!a_ctype(kb)) {
-            // A element (m,k) at A[m + k*lda], M-contiguous
+        const bool act = a_ctype(kb);
 #pragma unroll
-            for (int it = 0; it < BM * BK / NT; ++it) {
-                const int idx = tid + it * NT;
-                const int m = idx % BM, k = idx / BM;
-                const int gm = m0 + m, gk = k0 + k;
-                const bool ok = gm < p.M && gk < Kp;
-                const c128* src = ok ? A + gm + (int64_t)gk * lda : A;
-                cp_async16(As + k * Cfg::SA_N + m, src, ok ? 16 : 0);
-            }
-        } else {
-            // A element (m,k) = conj(A[k + m*lda]), K-contiguous
-#pragma unroll
-            for (int it = 0; it < BM * BK / NT; ++it) {
-                const int idx = tid + it * NT;
-                const int k = idx % BK, m = idx / BK;
-                const int gm = m0 + m, gk = k0 + k;
-                const bool ok = gm < p.M && gk < Kp;
-                const c128* src = ok ? A + gk + (int64_t)gm * lda : A;
-                cp_async16(As + m * ZG_KSTRIDE + k, src, ok ? 16 : 0);
-            }
+        for (int it = 0; it < NA; ++it) {
+            const int idx = tid + it * NT;
+            int m, k;
+            if (!act) { m = idx % BM; k = idx / BM; }        // A element (m,k) at A[m + k*lda], M-contiguous
+            else      { k = idx % BK; m = idx / BK; }        // A element (m,k) = conj(A[k + m*lda]), K-contiguous
+            const int gm = m0 + m;
+            vA[it] = gm < p.M;
+            kA[it] = k;
+            pA[it] = !act ? A + gm + (int64_t)(k0 + k) * lda : A + (k0 + k) + (int64_t)gm * lda;
+            sA[it] = !act ? k * Cfg::SA_N + m : m * ZG_KSTRIDE + k;
         }
-        if (!TB) {
-            // B element (k,n) at B[k + n*ldb], K-contiguous
+        dA = !act ? (int64_t)BK * lda : BK;
 #pragma unroll
-            for (int it = 0; it < BN * BK / NT; ++it) {
-                const int idx = tid + it * NT;
-                const int k = idx % BK, n = idx / BK;
-                const int gn = n0 + n, gk = k0 + k;
-                const bool ok = gn < p.N && gk < Kp;
-                const c128* src = ok ? B + gk + (int64_t)gn * ldb : B;
-                cp_async16(Bs + n * ZG_KSTRIDE + k, src, ok ? 16 : 0);
-            }
-        } else {
-            // B element (k,n) = conj(B[n + k*ldb]), N-contiguous
-#pragma unroll
-            for (int it = 0; it < BN * BK / NT; ++it) {
-                const int idx = tid + it * NT;
-                const int n = idx % BN, k = idx / BN;
-                const int gn = n0 + n, gk = k0 + k;
-                const bool ok = gn < p.N && gk < Kp;
-                const c128* src = ok ? B + gn + (int64_t)gk * ldb : B;
-                cp_async16(Bs + k * Cfg::SB_C + n, src, ok ? 16 : 0);
-            }
+        for (int it = 0; it < NB; ++it) {
+            const int idx = tid + it * NT;
+            int n, k;
+            if (!TB) { k = idx % BK; n = idx / BK; }         // B element (k,n) at B[k + n*ldb], K-contiguous
+            else     { n = idx % BN; k = idx / BN; }         // B element (k,n) = conj(B[n + k*ldb]), N-contiguous
+            const int gn = n0 + n;
+            vB[it] = gn < p.N;
+            kB[it] = k;
+            pB[it] = !TB ? B + (k0 + k) + (int64_t)gn * ldb : B + gn + (int64_t)(k0 + k) * ldb;
+            sB[it] = !TB ? n * ZG_KSTRIDE + k : k * Cfg::SB_C + n;
         }
+        dB = !TB ? BK : (int64_t)BK * ldb;
+        ld_krem = Kp - k0;
+        ld_switch = 0x7fffffff;
+        if (!second && nkb2 > 0) ld_switch = nkb1;
+        if (MODE == ZMODE_HEMM && !act) ld_switch = min(ld_switch, (m0 + BM) / BK);
+    };
+    auto load_next = [&](int stage) {          // requests block ld_kb into `stage`
+        if (ld_kb == ld_switch) ld_setup(ld_kb);
+        c128* As = smem + (size_t)stage * Cfg::STAGE;
+        c128* Bs = As + Cfg::A_STAGE;
+#pragma unroll
+        for (int it = 0; it < NA; ++it) {
+            const bool ok = vA[it] && kA[it] < ld_krem;
+            cp_async16(As + sA[it], ok ? pA[it] : ld_safe, ok ? 16 : 0);
+            pA[it] += dA;
+        }
+#pragma unroll
+        for (int it = 0; it < NB; ++it) {
+            const bool ok = vB[it] && kB[it] < ld_krem;
+            cp_async16(Bs + sB[it], ok ? pB[it] : ld_safe, ok ? 16 : 0);
+            pB[it] += dB;
+        }
+        ld_krem -= BK;
+        ++ld_kb;
     };
 
     // prologue
 #pragma unroll
     for (int s = 0; s < ZG_STAGES - 1; ++s) {
-        if (kb_begin + s < kb_end) load_stage(s, kb_begin + s);
+        if (kb_begin + s < kb_end) load_next(s);
         cp_async_commit();
     }
     for (int kb = kb_begin; kb < kb_end; ++kb) {
@@ -262,7 +276,7 @@ __global__ void __launch_bounds__(32 * WARPS_M * WARPS_N, MINB) zgemm_kernel(con
         __syncthreads();
         {
             const int nxt = kb + ZG_STAGES - 1;
-            if (nxt < kb_end) load_stage((nxt - kb_begin) % ZG_STAGES, nxt);
+            if (nxt < kb_end) load_next((nxt - kb_begin) % ZG_STAGES);
             cp_async_commit();
         }
         const int stage = (kb - kb_begin) % ZG_STAGES;
