@@ -66,38 +66,58 @@ static __global__ void __launch_bounds__(DG_NT, 1) dgemm_kernel(const DgemmArgs 
 
     const int nkb = (d.K + DG_BK - 1) / DG_BK;
 
+    // Per-thread loader state (fixed over the k-blocks): row pair / k of its A elements, column / k pair of its B
+    // elements, their shared-memory slots; only the gathered column of A and the B pointer change from block to block.
+    constexpr int NA = DG_BM * DG_BK / 2 / DG_NT, NB = DG_BN * DG_BK / 2 / DG_NT;
+    const double* pA[NA];
+    const double* pB[NB];
+    int kA[NA], sA[NA], bA[NA], kB[NB], sB[NB];
+    bool vB[NB];
+#pragma unroll
+    for (int it = 0; it < NA; ++it) {
+        const int idx = tid + it * DG_NT;
+        const int mp = idx % (DG_BM / 2), k = idx / (DG_BM / 2);
+        const int gm = m0 + 2 * mp;
+        kA[it] = k;
+        sA[it] = k * DG_SA + 2 * mp;
+        bA[it] = gm >= d.M ? 0 : (gm + 1 < d.M ? 16 : 8);
+        pA[it] = A + (gm < d.M ? gm : 0);
+    }
+#pragma unroll
+    for (int it = 0; it < NB; ++it) {
+        const int idx = tid + it * DG_NT;
+        const int kp = idx % (DG_BK / 2), n = idx / (DG_BK / 2);
+        const int gn = n0 + n;
+        kB[it] = 2 * kp;
+        sB[it] = n * DG_SB + 2 * kp;
+        vB[it] = gn < d.N;
+        pB[it] = B + 2 * kp + (int64_t)(gn < d.N ? gn : 0) * p.ldb;
+    }
     auto load_stage = [&](int stage, int kb) {
         double* As = smem + (size_t)stage * DG_STAGE;
         double* Bs = As + DG_BK * DG_SA;
         const int k0 = kb * DG_BK;
-        // A: pairs along m.  BM*BK/2 = 1024 pairs, 4 per thread
+        const int krem = d.K - k0;
 #pragma unroll
-        for (int it = 0; it < DG_BM * DG_BK / 2 / DG_NT; ++it) {
-            const int idx = tid + it * DG_NT;
-            const int mp = idx % (DG_BM / 2), k = idx / (DG_BM / 2);
-            const int gm = m0 + 2 * mp, gk = k0 + k;
+        for (int it = 0; it < NA; ++it) {
             int bytes = 0;
             const double* src = A;
-            if (gk < d.K && gm < d.M) {
-                const int64_t col = cidx ? (int64_t)__ldg(cidx + gk) : (int64_t)gk;
-                src = A + gm + col * p.lda;
-                bytes = (gm + 1 < d.M) ? 16 : 8;
+            if (kA[it] < krem && bA[it]) {
+                const int64_t col = cidx ? (int64_t)__ldg(cidx + k0 + kA[it]) : (int64_t)(k0 + kA[it]);
+                src = pA[it] + col * p.lda;
+                bytes = bA[it];
             }
-            cp_async16(As + k * DG_SA + 2 * mp, src, bytes);
+            cp_async16(As + sA[it], src, bytes);
         }
-        // B: pairs along k.  BN*BK/2 = 1024 pairs
 #pragma unroll
-        for (int it = 0; it < DG_BN * DG_BK / 2 / DG_NT; ++it) {
-            const int idx = tid + it * DG_NT;
-            const int kp = idx % (DG_BK / 2), n = idx / (DG_BK / 2);
-            const int gn = n0 + n, gk = k0 + 2 * kp;
+        for (int it = 0; it < NB; ++it) {
             int bytes = 0;
             const double* src = B;
-            if (gn < d.N && gk < d.K) {
-                src = B + gk + (int64_t)gn * p.ldb;
-                bytes = (gk + 1 < d.K) ? 16 : 8;
+            if (vB[it] && kB[it] < krem) {
+                src = pB[it] + k0;
+                bytes = (kB[it] + 1 < krem) ? 16 : 8;
             }
-            cp_async16(Bs + n * DG_SB + 2 * kp, src, bytes);
+            cp_async16(Bs + sB[it], src, bytes);
         }
     };
 
