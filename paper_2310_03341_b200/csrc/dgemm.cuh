@@ -28,13 +28,13 @@ struct DgemmArgs {
     DgemmDesc one;
 };
 
-constexpr int DG_BM = 128, DG_BN = 128, DG_BK = 16, DG_STAGES = 4, DG_NT = 256;
+constexpr int DG_BM = 128, DG_BN = 64, DG_BK = 16, DG_STAGES = 4, DG_NT = 256;   // 108 KB of shared memory: 2 thread blocks per SM
 constexpr int DG_SA = DG_BM + 4;     // As[k][m], stride == 4 (mod 16) doubles
 constexpr int DG_SB = DG_BK + 4;     // Bs[n][k]
 constexpr int DG_STAGE = DG_BK * DG_SA + DG_BN * DG_SB;    // doubles
 constexpr size_t DG_SMEM_BYTES = (size_t)DG_STAGES * DG_STAGE * sizeof(double);
 
-static __global__ void __launch_bounds__(DG_NT, 1) dgemm_kernel(const DgemmArgs p) {
+static __global__ void __launch_bounds__(DG_NT, 2) dgemm_kernel(const DgemmArgs p) {
     extern __shared__ __align__(16) unsigned char dg_smem_raw[];
     double* smem = reinterpret_cast<double*>(dg_smem_raw);
 
@@ -56,11 +56,11 @@ static __global__ void __launch_bounds__(DG_NT, 1) dgemm_kernel(const DgemmArgs 
 
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int g = lane >> 2, t = lane & 3;
-    const int wm0 = (warp & 1) * 64, wn0 = (warp >> 1) * 32;   // 2 x 4 warps, warp tile 64 x 32
+    const int wm0 = (warp & 3) * 32, wn0 = (warp >> 2) * 32;   // 4 x 2 warps, warp tile 32 x 32
 
-    double acc[8][4][2];
+    double acc[4][4][2];
 #pragma unroll
-    for (int i = 0; i < 8; ++i)
+    for (int i = 0; i < 4; ++i)
 #pragma unroll
         for (int j = 0; j < 4; ++j) acc[i][j][0] = acc[i][j][1] = 0.0;
 
@@ -138,13 +138,13 @@ static __global__ void __launch_bounds__(DG_NT, 1) dgemm_kernel(const DgemmArgs 
         const double* Bs = As + DG_BK * DG_SA;
 #pragma unroll
         for (int kk = 0; kk < DG_BK; kk += 4) {
-            double a[8], b[4];
+            double a[4], b[4];
 #pragma unroll
-            for (int i = 0; i < 8; ++i) a[i] = As[(kk + t) * DG_SA + wm0 + 8 * i + g];
+            for (int i = 0; i < 4; ++i) a[i] = As[(kk + t) * DG_SA + wm0 + 8 * i + g];
 #pragma unroll
             for (int j = 0; j < 4; ++j) b[j] = Bs[(wn0 + 8 * j + g) * DG_SB + kk + t];
 #pragma unroll
-            for (int i = 0; i < 8; ++i)
+            for (int i = 0; i < 4; ++i)
 #pragma unroll
                 for (int j = 0; j < 4; ++j) dmma884p(acc[i][j][0], acc[i][j][1], a[i], b[j]);
         }
@@ -152,7 +152,7 @@ static __global__ void __launch_bounds__(DG_NT, 1) dgemm_kernel(const DgemmArgs 
     cp_async_wait<0>();
 
 #pragma unroll
-    for (int i = 0; i < 8; ++i) {
+    for (int i = 0; i < 4; ++i) {
         const int row = m0 + wm0 + 8 * i + g;
 #pragma unroll
         for (int j = 0; j < 4; ++j)
