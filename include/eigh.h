@@ -213,6 +213,13 @@ int eigh_k_dgemm(eigh_handle_t h, int64_t M, int64_t N, int64_t K, const double*
  * instructions per thread on every SM; returns achieved real TFLOP/s in *tflops (host). */
 int eigh_k_fp64_peak(int use_dmma, int64_t iters, double* tflops, double* ms, void* stream);
 
+/* Configurable variant: kind 0 = DFMA loop, 1 = mma.sync.m8n8k4.f64 loop, 2 = mma.sync.m16n8k16.f64 loop, with
+ * `blocks_per_sm` thread blocks of `threads` threads on every SM; kind 10..13 = the inner loop of the 3M GEMM engine
+ * (10: DMMAs on register operands, 11: + shared-memory fragment loads and the 3M adds, 12: + a block barrier per k-block,
+ * 13: + the cp.async traffic of a k-block; fixed at 3 blocks of 128 threads per SM).  Returns real TFLOP/s (2 per FMA). */
+int eigh_k_fp64_probe(int kind, int blocks_per_sm, int threads, int64_t iters, double* tflops, double* ms,
+                      void* stream);
+
 #ifdef __cplusplus
 }
 #endif

@@ -44,6 +44,7 @@ SIGNATURES = {
     "eigh_k_zhemm_lower": (_int, [_vp, _i64, _i64, _vp, _i64, _vp, _i64, _vp, _i64, _int, _vp]),
     "eigh_k_dgemm": (_int, [_vp, _i64, _i64, _i64, _vp, _i64, _vp, _vp, _i64, _vp, _i64, _vp]),
     "eigh_k_fp64_peak": (_int, [_int, _i64, _dp, _dp, _vp]),
+    "eigh_k_fp64_probe": (_int, [_int, _int, _int, _i64, _dp, _dp, _vp]),
 }
 
 
@@ -278,4 +279,15 @@ def fp64_peak(use_dmma: bool, iters: int = 20000):
     rc = lib.eigh_k_fp64_peak(1 if use_dmma else 0, iters, ctypes.byref(tf), ctypes.byref(ms), _stream())
     if rc != 0:
         raise EighError(f"eigh_k_fp64_peak -> {rc}")
+    return tf.value, ms.value
+
+
+def fp64_probe(kind: int, blocks_per_sm: int = 2, threads: int = 256, iters: int = 20000):
+    """(TFLOP/s, ms) of one configuration of the FP64 microbenchmarks (eigh_k_fp64_probe)."""
+    lib = load()
+    tf, ms = ctypes.c_double(), ctypes.c_double()
+    rc = lib.eigh_k_fp64_probe(int(kind), int(blocks_per_sm), int(threads), int(iters), ctypes.byref(tf), ctypes.byref(ms),
+                               _stream())
+    if rc != 0:
+        raise EighError(f"eigh_k_fp64_probe -> {rc}")
     return tf.value, ms.value

@@ -459,68 +459,3 @@ int eigh_k_dgemm(eigh_handle_t h, int64_t M, int64_t N, int64_t K, const double*
 
 }  // extern "C"
 
-// ------------------------------------------------------------------------- FP64 peak microbenchmarks
-namespace eigh {
-__global__ void __launch_bounds__(256) peak_dmma_kernel(int64_t iters, double* sink) {
-    double c[16][2];
-#pragma unroll
-    for (int i = 0; i < 16; ++i) { c[i][0] = 0.0; c[i][1] = 0.0; }
-    const double a = 1.0 + 1e-9 * threadIdx.x, b = 1.0 - 1e-9 * threadIdx.x;
-    for (int64_t it = 0; it < iters; ++it) {
-#pragma unroll
-        for (int i = 0; i < 16; ++i) dmma884(c[i][0], c[i][1], a, b);
-    }
-    double s = 0.0;
-#pragma unroll
-    for (int i = 0; i < 16; ++i) s += c[i][0] + c[i][1];
-    if (s == 123.456) sink[0] = s;
-}
-__global__ void __launch_bounds__(256) peak_dfma_kernel(int64_t iters, double* sink) {
-    double c[16];
-#pragma unroll
-    for (int i = 0; i < 16; ++i) c[i] = 1e-3 * i;
-    const double a = 1.0 + 1e-9 * threadIdx.x, b = 1e-9 * threadIdx.x;
-    for (int64_t it = 0; it < iters; ++it) {
-#pragma unroll
-        for (int i = 0; i < 16; ++i) c[i] = fma(c[i], a, b);
-    }
-    double s = 0.0;
-#pragma unroll
-    for (int i = 0; i < 16; ++i) s += c[i];
-    if (s == 123.456) sink[0] = s;
-}
-}  // namespace eigh
-
-extern "C" int eigh_k_fp64_peak(int use_dmma, int64_t iters, double* tflops, double* ms_out, void* stream) {
-    if (iters < 1) return -2;
-    if (!tflops) return -3;
-    cudaStream_t s = (cudaStream_t)stream;
-    int dev = 0, sms = 0;
-    EIGH_CUDA_OK(cudaGetDevice(&dev));
-    EIGH_CUDA_OK(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
-    double* sink = nullptr;
-    EIGH_CUDA_OK(cudaMalloc(&sink, 8));
-    cudaEvent_t e0, e1;
-    EIGH_CUDA_OK(cudaEventCreate(&e0));
-    EIGH_CUDA_OK(cudaEventCreate(&e1));
-    const int blocks = sms * 4, threads = 256;
-    for (int rep = 0; rep < 2; ++rep) {   // first pass = warm-up
-        EIGH_CUDA_OK(cudaEventRecord(e0, s));
-        if (use_dmma) eigh::peak_dmma_kernel<<<blocks, threads, 0, s>>>(iters, sink);
-        else eigh::peak_dfma_kernel<<<blocks, threads, 0, s>>>(iters, sink);
-        EIGH_CUDA_OK(cudaGetLastError());
-        EIGH_CUDA_OK(cudaEventRecord(e1, s));
-        EIGH_CUDA_OK(cudaEventSynchronize(e1));
-    }
-    float ms = 0.f;
-    EIGH_CUDA_OK(cudaEventElapsedTime(&ms, e0, e1));
-    const double warps = (double)blocks * threads / 32.0;
-    const double flops = use_dmma ? warps * (double)iters * 16.0 * 512.0
-                                  : (double)blocks * threads * (double)iters * 16.0 * 2.0;
-    *tflops = flops / (ms * 1e-3) / 1e12;
-    if (ms_out) *ms_out = ms;
-    cudaEventDestroy(e0);
-    cudaEventDestroy(e1);
-    cudaFree(sink);
-    return 0;
-}

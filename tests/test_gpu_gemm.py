@@ -129,6 +129,14 @@ def test_fp64_peak_and_gemm_rate(eng):
     out["dmma_tflops_sustained"] = tf
     out["dmma_sustained_ms"] = ms
 
+    # DMMA rate against the number of resident warps per SM sub-partition, and the cost of the ingredients of the GEMM
+    # engine's inner loop (eigh_k_fp64_probe; profiles/r01_fp64_peaks.md)
+    for wps, (bps, thr) in {1: (1, 128), 2: (1, 256), 3: (1, 384), 4: (2, 256), 8: (4, 256)}.items():
+        out[f"dmma_tflops_{wps}_warps_per_smsp"] = binding.fp64_probe(1, bps, thr, 20000)[0]
+    out["dmma_m16n8k16_tflops_8_warps_per_smsp"] = binding.fp64_probe(2, 4, 256, 2500)[0]
+    for mode, name in ((10, "dmma_only"), (11, "lds_and_3m_adds"), (12, "barrier"), (13, "cp_async")):
+        out[f"gemm_loop_tflops_{name}"] = binding.fp64_probe(mode, 3, 128, 20000)[0]
+
     def timeit(fn, n=5):
         fn()
         torch.cuda.synchronize()
