@@ -118,7 +118,7 @@ int eigh_set_option(eigh_handle_t h, const char* key, int64_t value) {
         if (value < 4 || value > 32) return set_err(h, -3, "dc_leaf must be in [4, 32]");
         h->leaf = (int)value;
     } else if (!strcmp(key, "p4b_merge")) {
-        if (value < 1 || value > 4) return set_err(h, -3, "p4b_merge must be in [1, 4]");
+        if (value < 1 || value > 8) return set_err(h, -3, "p4b_merge must be in [1, 8]");
         h->p4b_merge = (int)value;
     } else if (!strcmp(key, "gemm_3m")) {
         if (value != 0 && value != 1) return set_err(h, -3, "gemm_3m must be 0 or 1");
