@@ -120,3 +120,16 @@ def test_degenerate_inputs():
     W, Z, _ = gpu_solve(I)
     assert np.abs(W - 2.5).max() <= 1e-14
     assert np.abs(Z.conj().T @ Z - np.eye(N)).max() <= 1e-12 * N
+
+
+@pytest.mark.parametrize("N", [130, 257, 389])
+@pytest.mark.parametrize("nev_of", [lambda N: 1, lambda N: 7, lambda N: 63, lambda N: 65, lambda N: N - 1])
+def test_ragged_subsets(N, nev_of):
+    """Odd N with odd nev: ragged tiles in every GEMM of S3 / S4a / S4b (N-tails of 1, 7, 63, 65 columns), the column
+    slabs of S4a with a partial last slab, and the nev-aware last merge of S3."""
+    nev = nev_of(N)
+    H = rand_herm(N, 5000 + N)
+    W, Z, _ = gpu_solve(H, nev=nev)
+    assert Z.shape == (N, nev)
+    Wo = oracle.eigh(H, vectors=False)
+    check(H, W, Z, Wo, nev=nev)
