@@ -188,6 +188,9 @@ def main():
     ap.add_argument("--cpu-sample", type=int, default=1024)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--context", action="store_true",
+                    help="also time library routines on the same matrix as CONTEXT (never the target, never on the hot path): "
+                         "torch.linalg.eigh (cuSOLVER) on this GPU and numpy.linalg.eigh (LAPACK) on the CPU sample")
     ap.add_argument("--wy-group", type=int, default=0)
     ap.add_argument("--opt", action="append", default=[], help="solver option key=value (eigh_set_option), repeatable")
     args = ap.parse_args()
@@ -404,6 +407,33 @@ def main():
         cpu = {"value": dt * (N / ns) ** 3, "unit": "s", "cores": oracle.num_threads(), "kind": "oracle",
                "sample": f"leading {ns}x{ns} block: {dt:.3f} s measured, scaled by (N/{ns})^3 (23 N^3 flops method)"}
 
+    # ---- context rows: library eigensolvers on the same seeded matrix; reported, never the target
+    context = None
+    if args.context and rank == 0 and world == 1:
+        context = {}
+        try:
+            del Zt
+            torch.cuda.empty_cache()
+            Hc = w.dense_torch(dev, out=At)                   # logical H (column-major storage in At)
+            torch.cuda.synchronize()
+            ev0.record(stream)
+            Wc, Zc = torch.linalg.eigh(Hc)
+            ev1.record(stream)
+            torch.cuda.synchronize()
+            context["torch_linalg_eigh_s"] = ev0.elapsed_time(ev1) / 1e3
+            context["torch_linalg_eigh_max_abs_diff_W"] = float((Wc - W).abs().max().item())
+            del Wc, Zc
+        except Exception as ex:
+            context["torch_linalg_eigh_error"] = str(ex)[:200]
+        try:
+            ns = min(N, args.cpu_sample)
+            Hs = _leading_block_bdg(w, ns) if w.problem is not None else w.dense()[:ns, :ns]
+            tt = time.perf_counter()
+            np.linalg.eigh(Hs)
+            context["numpy_linalg_eigh_sample"] = {"n": ns, "s": time.perf_counter() - tt}
+        except Exception as ex:
+            context["numpy_linalg_eigh_error"] = str(ex)[:200]
+
     if rank != 0:
         if dist is not None:
             dist.destroy_process_group()
@@ -468,7 +498,7 @@ def main():
                    "l2": "inputs larger than L2 (matrix %.1f GB)" % (mat_bytes / 1e9),
                    "input_regeneration": "device copy outside the timed brackets"},
         "clocks": clocks, "e2e": e2e, "gpu_launches": launches, "phases": phase_report, "roofline": roofline,
-        "cpu_baseline": cpu, "validity": valid, "epilogue": epilogue,
+        "cpu_baseline": cpu, "validity": valid, "epilogue": epilogue, "context": context,
         "total_tflops": (cw["p1_flops"] + cw["p2_flops"] + cw["p4a_flops"] + cw["p4b_flops"]) / ms_per_step / 1e9,
     }
     print(json.dumps(line))
