@@ -150,7 +150,7 @@ __device__ __forceinline__ c128 bc_make_reflector(c128 x, const BcStepCtx& t, in
 // One chase step (sweep j, step k) by the compute group.  FULL: len = len2 = 64 (no edge predicates).
 // Returns false when the sweep ended with this step (no S block below).
 template <bool FULL>
-__device__ __forceinline__ bool bc_step(BcSmem& sm, const BcStepCtx& t, int r0, int len_, int len2_, int k, c128& tau) {
+__device__ __forceinline__ bool bc_step(BcSmem& sm, const BcStepCtx& t, int r0, int len_, int len2_, int k, c128& tau, int& hb) {
     const int len = FULL ? BC_B : len_, len2 = FULL ? BC_B : len2_;
     const int r = t.r, q = t.q, rl = t.rl;
     c128* const band = t.band;
@@ -270,6 +270,13 @@ __device__ __forceinline__ bool bc_step(BcSmem& sm, const BcStepCtx& t, int r0, 
             }
         }
     }
+    // ---- early hand-off.  The next sweep's step k-1 overlaps this step's blocks only in the first column of D_k (stored
+    //      above) and in S_{k+1}(0,0) = beta' (stored here); everything else it reads was final one step ago.  So the
+    //      release of "step k" is handed to the publisher warp now, and the rest of the step (left update of S_{k+1}, its
+    //      stores, the reflector) runs behind it: the lag between consecutive sweeps drops from 2 steps to ~1.6.
+    if (has_s && r == 0 && q == 0) band[BC_B + (int64_t)r0 * ldab] = cmake(betan, 0.0);
+    bc_handoff_arrive(hb);
+    hb ^= 1;
     if (!has_s) return false;
     BC_STAMP(5);
     // ---- z_c = vn^H S[:, c]: per-thread products, reduce-scatter over the 8 row lanes, then across warps
@@ -317,7 +324,8 @@ __device__ __forceinline__ bool bc_step(BcSmem& sm, const BcStepCtx& t, int r0, 
                 e.x -= vnr.x * zc.x - vnr.y * zc.y;
                 e.y -= vnr.x * zc.y + vnr.y * zc.x;
             }
-            if (FULL || (r < len2 && c < len)) sp[(int64_t)i * 4 * (ldab - 1)] = e;
+            // (0,0) was stored before the hand-off and may already have been updated by the next sweep
+            if ((FULL || (r < len2 && c < len)) && !(c == 0 && r == 0)) sp[(int64_t)i * 4 * (ldab - 1)] = e;
         }
     }
     if (q == 0) {
@@ -338,7 +346,8 @@ __global__ void __launch_bounds__(BC_NT + 32, 1) bulge_chase_kernel(const BcArgs
     const int N = a.N;
 
     if (warp == BC_NW) {
-        // ================= publisher warp: one release per completed step, INT_MAX per completed sweep
+        // ================= publisher warp: one release per step whose D phase is complete (the previous step is then
+        // complete in full), INT_MAX per completed sweep
         int hb = 0;
         for (int j = blockIdx.x; j <= N - 2; j += gridDim.x) {
             for (int k = 0;; ++k) {
@@ -386,11 +395,9 @@ __global__ void __launch_bounds__(BC_NT + 32, 1) bulge_chase_kernel(const BcArgs
             const int r0 = j + 1 + k * BC_B;
             const int len = min(BC_B, N - r0);
             const int len2 = min(BC_B, N - (r0 + BC_B));
-            const bool more = (len == BC_B && len2 == BC_B) ? bc_step<true>(sm, t, r0, len, len2, k, tau)
-                                                            : bc_step<false>(sm, t, r0, len, len2, k, tau);
-            // all band / reflector stores of this step are issued: hand the release to the publisher warp
-            bc_handoff_arrive(hb);
-            hb ^= 1;
+            // (the release of the step is handed to the publisher warp inside bc_step, after the D phase)
+            const bool more = (len == BC_B && len2 == BC_B) ? bc_step<true>(sm, t, r0, len, len2, k, tau, hb)
+                                                            : bc_step<false>(sm, t, r0, len, len2, k, tau, hb);
             if (!more) break;
             if (tid == 0) bc_poll(a.progress, j - 1, k + 3);
             bc_sync_compute();
