@@ -220,6 +220,9 @@ __device__ __forceinline__ void dmma_p(double (&c)[2], double a, double b) {
 #ifndef BT_GAUSS2
 #define BT_GAUSS2 1
 #endif
+#ifndef BT_3M1
+#define BT_3M1 1
+#endif
 
 struct BtSweepArgs {
     c128* Z; int64_t ldz;
@@ -277,9 +280,17 @@ __device__ __forceinline__ void bt_apply_step(const c128* __restrict__ Vs, const
                         c128 v = cmake(0.0, 0.0);
                         if ((p != cb || 2 * t + h >= g) && (p != cb + 8 || 2 * t + h < g))
                             v = Vs[(8 * p + 2 * t + h) + (8 * cb + g) * BT_LDV];
+#if BT_3M1
                         dmma_p(s1[c][h], ar, v.x);
                         dmma_p(s2[c][h], ai, v.y);
                         dmma_p(s3[c][h], as, v.x - v.y);
+#else
+                        // four products: s1 = Re = sum ar vx + ai vy,  s3 = Im = sum ai vx - ar vy  (s2 stays zero)
+                        dmma_p(s1[c][h], ar, v.x);
+                        dmma_p(s1[c][h], ai, v.y);
+                        dmma_p(s3[c][h], ai, v.x);
+                        dmma_p(s3[c][h], ar, -v.y);
+#endif
                     }
                 }
             }
@@ -290,8 +301,13 @@ __device__ __forceinline__ void bt_apply_step(const c128* __restrict__ Vs, const
 #pragma unroll
             for (int e = 0; e < 2; ++e) {
                 const double t1 = s1[c][0][e] + s1[c][1][e], t2 = s2[c][0][e] + s2[c][1][e], t3 = s3[c][0][e] + s3[c][1][e];
+#if BT_3M1
                 ar1[c][e] = t1 + t2;
                 ai1[c][e] = (t3 - t1) + t2;
+#else
+                ar1[c][e] = t1 + t2;          // t2 = 0
+                ai1[c][e] = t3;
+#endif
             }
         // ---- Y = (-T) Y1   (m = column of Z, n = output reflector, k = input reflector >= output)
         double yr[NB][2], yi[NB][2];
