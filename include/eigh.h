@@ -46,6 +46,7 @@ int eigh_create(eigh_handle_t* h, int64_t N, int64_t nev);
  * multiply-add, the default; 0 = four products.  The switch is process-wide: handles used concurrently must agree),
  * "panel_smem" (S1.1: 1 = shared-memory resident panel QR with the T factor built in, 0 = L2-resident panel QR + Gram
  * GEMM + T recurrence), "panel_rows_min" (16..192 panel rows per thread block of the resident kernel),
+ * "hemm_waves" (S1.3: split-K of HEMM-lower sized for about this many thread blocks per SM; default 14, 7..28 measure within 1 %),
  * "bt_chain" (S4a: consecutive passes of one column slab scheduled back to back so that followers read from L2;
  * 0 = automatic = 1, the unchained order, which measures fastest), "bc_grid" (thread blocks of the S2 bulge-chasing kernel; 0 = every co-resident block, the default).
  * Returns -2 for an unknown key, -3 for a bad value. */

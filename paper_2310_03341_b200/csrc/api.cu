@@ -99,6 +99,7 @@ int eigh_create(eigh_handle_t* out, int64_t N, int64_t nev) {
     h->gemm_3m = 1;
     h->panel_smem = 1;
     h->panel_rows_min = 96;
+    h->hemm_waves = 14;
     h->num_sms = 0;
     snprintf(h->err, sizeof(h->err), "ok");
     *out = h;
@@ -132,6 +133,9 @@ int eigh_set_option(eigh_handle_t h, const char* key, int64_t value) {
     } else if (!strcmp(key, "bt_chain")) {
         if (value < 0 || value > 16) return set_err(h, -3, "bt_chain must be in [0, 16]");
         h->bt_chain = (int)value;
+    } else if (!strcmp(key, "hemm_waves")) {
+        if (value < 1 || value > 64) return set_err(h, -3, "hemm_waves must be in [1, 64]");
+        h->hemm_waves = (int)value;
     } else if (!strcmp(key, "bc_grid")) {
         if (value < 0 || value > 4096) return set_err(h, -3, "bc_grid must be in [0, 4096]");
         h->bc_grid = (int)value;

@@ -546,7 +546,7 @@ int phase_reduce_to_band(eigh_handle_s* h, c128* A, int64_t lda, c128* band, int
         // S1.3 X = Herm(A22) VT
         {
             const int tiles = (int)ceil_div(m, 64);
-            int sk = (int)ceil_div(14 * h->num_sms, tiles);
+            int sk = (int)ceil_div((int64_t)h->hemm_waves * h->num_sms, tiles);
             if (sk > 16) sk = 16;
             if (m / sk < 512) sk = max(1, m / 512);
             rc = zg(h, false, false, m, b, m, 1.0, A22, lda, VT, m, 0.0, X, m, true, sk, s, 0, 0, nullptr, 0, nullptr,

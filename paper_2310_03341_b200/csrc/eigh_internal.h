@@ -44,6 +44,7 @@ struct eigh_handle_s {
     int gemm_3m;         // complex GEMMs by the 3M method (1) or with four real products (0)
     int panel_smem;      // S1.1: shared-memory resident panel QR (1) or the L2-resident one (0)
     int panel_rows_min;  // S1.1: fewest panel rows per thread block of the resident kernel
+    int hemm_waves;      // S1.3: split-K of HEMM-lower chosen for about this many thread blocks per SM
     int bt_chain;   // S4a: consecutive passes of one slab scheduled back to back (0 = auto)
     int bc_grid;    // S2: CTAs of the bulge-chasing kernel (0 = all that are co-resident)
     int64_t ldab;   // band storage leading dimension
