@@ -178,6 +178,29 @@ def test_config3_densities_from_the_lowest_half():
     torch.cuda.synchronize()
     assert float((n - 1.0).abs().max().item()) <= 1e-9
     assert float(nu.abs().max().item()) <= 1e-9
+    # Eq. 16b / 16c at the same size, EVERY grid point: the oracle needs whole states for the gradients, so the 2048
+    # lowest-|E| states are taken (columns nev-2048 .. nev-1, contiguous rows of Zt) and mapped to the positive branch
+    shape = w.problem.shape
+    Ds = [wl.derivative_1d(L) for L in shape]
+    Dd = [torch.from_numpy(np.ascontiguousarray(D.T)).to(dev) for D in Ds]
+    k = 2048
+    Zk = Zt[nev - k:]
+    Ek = E[nev - k:].contiguous()
+    tau, j = eng.gradient_densities(shape, Dd[0], Dd[1], Dd[2], Ek, Zk, T=0.05, branch=-1)
+    torch.cuda.synchronize()
+    Ep, Zp = od.particle_hole_map(Ek.cpu().numpy(), Zk.t().cpu().numpy())
+    tau_o, j_o = od.gradient_densities(Ep, Zp, shape, *Ds, T=0.05)
+    t_inf, _ = od.gradient_densities(np.ones(k), Zp, shape, *Ds, T=1e12)
+    n_inf, _ = od.densities(np.ones(k), Zp, T=1e12)
+    c = 8.0 * (k + 2 * max(shape)) * np.finfo(np.float64).eps
+    assert np.abs(tau.cpu().numpy() - tau_o).max() <= c * 2.0 * t_inf.max()
+    assert np.abs(j.cpu().numpy() - j_o).max() <= c * 2.0 * np.sqrt(t_inf.max() * n_inf.max())
+    # completeness over all N/2 states at T -> infinity: tau(r) = sum_a (D_a D_a^T)[i_a, i_a] (constant), j(r) = 0
+    tau, j = eng.gradient_densities(shape, Dd[0], Dd[1], Dd[2], E, Zt, T=1e12, branch=-1)
+    torch.cuda.synchronize()
+    ref = sum(float(np.sum(D * D, axis=1)[0]) for D in Ds)
+    assert float((tau - ref).abs().max().item()) <= 1e-8 * ref
+    assert float(j.abs().max().item()) <= 1e-8
     eng.close()
 
 
