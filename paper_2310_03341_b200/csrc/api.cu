@@ -31,6 +31,7 @@ size_t dc_arena_bytes(int64_t N);   // tridiag_dc.cu
 size_t dc_result_offset(int64_t N);
 size_t bt_scratch_bytes(const eigh_handle_s* h);   // bt_band.cu
 size_t bt_tneg_bytes(int64_t N);
+size_t bt_vq_bytes(int64_t N);
 
 void plan_workspace(eigh_handle_s* h) {
     WsPlan& p = h->plan;
@@ -60,6 +61,11 @@ void plan_workspace(eigh_handle_s* h) {
     // S4a keeps its T factors in the first two (dead by then) Q buffers of the D&C arena when they fit
     if (bt_tneg_bytes(N) <= dc_result_offset(N)) p.btT = p.dc;
     else p.btT = bump(off, bt_tneg_bytes(N));
+    {
+        const size_t tb = (bt_tneg_bytes(N) + 255) / 256 * 256, qb = bt_vq_bytes(N);
+        if (p.btT == p.dc && tb + qb <= dc_result_offset(N)) p.btQ = p.dc + tb;
+        else p.btQ = bump(off, qb ? qb : 256);
+    }
     p.Qt = p.dc + dc_result_offset(N);   // eigh_solve lets S3 write its result over the dead U buffer
     // back-transform scratch aliases the tail of the D&C arena (U and the dead Q buffer)
     p.bt_bytes = bt_scratch_bytes(h);

@@ -43,6 +43,12 @@
 
 namespace eigh {
 
+#ifndef BT_QPLANE
+#define BT_QPLANE 1      // stage tiles carry q = vx - vy (a third bulk copy, 16 KB): no V-side adds in the two 3-product forms
+#endif
+#ifndef BT_RING8
+#define BT_RING8 (BT_QPLANE ? 3 : 4)
+#endif
 constexpr int BT_B = 64;            // band width (reflector length)
 constexpr int BT_P = 32;            // sweeps per pass
 constexpr int BT_WR = BT_B + BT_P;  // window rows (96)
@@ -56,7 +62,8 @@ constexpr int BT_LDZ = BT_B + 1;            // 65, odd: per-warp staging of the 
 constexpr int BT_ZS = 8 * BT_LDZ;           // c128 per warp
 // compact -T of one (pass, k) step for WY blocks of GS reflectors: 32/GS blocks [GS x GS], ld GS+1
 __host__ __device__ constexpr int bt_tsz(int gs) { return BT_P * (gs + 1); }
-__host__ __device__ constexpr int bt_stages(int gs) { return gs == 8 ? 4 : 3; }
+__host__ __device__ constexpr bool bt_qplane(int gs) { return BT_QPLANE && gs == 8; }   // 16 / 32: no shared memory left for it
+__host__ __device__ constexpr int bt_stages(int gs) { return gs == 8 ? BT_RING8 : 3; }
 constexpr int BT_CWARPS = 8;                // warps per CTA (all of them consumers)
 constexpr int BT_NT = 32 * BT_CWARPS;
 constexpr int BT_SLAB = 8 * BT_CWARPS;      // 64 columns per unit
@@ -64,6 +71,7 @@ constexpr int BT_SLAB = 8 * BT_CWARPS;      // 64 columns per unit
 struct BtHeader { int j0, k, slab, flags, pass, nk_pred, pad0, pad1; };   // flags: 1 first step of unit, 2 last step, 4 terminate
 __host__ __device__ constexpr size_t bt_smem(int gs) {
     return (size_t)bt_stages(gs) * (BT_VS + bt_tsz(gs)) * sizeof(c128) + (size_t)BT_CWARPS * BT_ZS * sizeof(c128) +
+           (bt_qplane(gs) ? (size_t)bt_stages(gs) * BT_VS * sizeof(double) : 0) +
            bt_stages(gs) * sizeof(BtHeader) + (2 * bt_stages(gs) + BT_CWARPS) * sizeof(uint64_t) + 64;
 }
 
@@ -224,10 +232,21 @@ __device__ __forceinline__ void dmma_p(double (&c)[2], double a, double b) {
 #define BT_3M1 1
 #endif
 
+// q = Re v - Im v for every stored reflector element (the third operand of the 3-product forms, formed once here instead
+// of once per warp and use inside the sweep)
+__global__ void bt_vq_kernel(const c128* __restrict__ V2, double* __restrict__ q, int64_t n) {
+    for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x) {
+        const c128 v = V2[i];
+        q[i] = v.x - v.y;
+    }
+}
+size_t bt_vq_bytes(int64_t N) { return BT_QPLANE ? (size_t)(v2_total_stages(N) * BT_VS + 64) * sizeof(double) : 0; }
+
 struct BtSweepArgs {
     c128* Z; int64_t ldz;
     int N, nev;
     const c128* V2;
+    const double* V2q;                  // q = Re v - Im v of every element of V2 (same tile-major layout)
     const c128* Tneg;
     const int64_t* pass_off;
     int npass, nslabs, chain;
@@ -247,7 +266,8 @@ __device__ __forceinline__ void bt_st_release(int* p, int v) {
 // ------------------------------------------------------------------ the sweeper
 // One (pass, k) step on the register window.  GS = reflectors per compact-WY block (8, 16 or 32).
 template <int GS, int S_HI, int S_LO>
-__device__ __forceinline__ void bt_apply_step(const c128* __restrict__ Vs, const c128* __restrict__ Ts,
+__device__ __forceinline__ void bt_apply_step(const c128* __restrict__ Vs, const double* __restrict__ Qs,
+                                              const c128* __restrict__ Ts,
                                               double (&zr)[BT_NBLK][2], double (&zi)[BT_NBLK][2], int g, int t,
                                               bool tail, int nrows) {
     constexpr int NB = GS / 8;          // column blocks per WY block
@@ -278,12 +298,16 @@ __device__ __forceinline__ void bt_apply_step(const c128* __restrict__ Vs, const
                     if (p >= cb && p <= cb + 8) {
                         // window row R = 8p+2t+h, reflector c = 8cb+g: inside the parallelogram iff 0 <= R - c < 64
                         c128 v = cmake(0.0, 0.0);
-                        if ((p != cb || 2 * t + h >= g) && (p != cb + 8 || 2 * t + h < g))
+                        double qv = 0.0;
+                        if ((p != cb || 2 * t + h >= g) && (p != cb + 8 || 2 * t + h < g)) {
                             v = Vs[(8 * p + 2 * t + h) + (8 * cb + g) * BT_LDV];
+                            if constexpr (bt_qplane(GS)) qv = Qs[(8 * p + 2 * t + h) + (8 * cb + g) * BT_LDV];
+                        }
+                        if constexpr (!bt_qplane(GS)) qv = v.x - v.y;
 #if BT_3M1
                         dmma_p(s1[c][h], ar, v.x);
                         dmma_p(s2[c][h], ai, v.y);
-                        dmma_p(s3[c][h], as, v.x - v.y);
+                        dmma_p(s3[c][h], as, qv);
 #else
                         // four products: s1 = Re = sum ar vx + ai vy,  s3 = Im = sum ai vx - ar vy  (s2 stays zero)
                         dmma_p(s1[c][h], ar, v.x);
@@ -327,6 +351,39 @@ __device__ __forceinline__ void bt_apply_step(const c128* __restrict__ Vs, const
                 }
         }
         // ---- Z += Y V   (m = column of Z, n = row, k = reflector)
+        if constexpr (bt_qplane(GS)) {
+        // Three real products per complex multiply-add with the precomputed q = vx - vy:  with y = ar + i ai,
+        //   k1 = ai q,  k2 = (ar - ai) vx,  k3 = (ar + ai) vy;   Re(y v) = k2 + k1,  Im(y v) = k3 + k1.
+#pragma unroll
+        for (int c = 0; c < NB; ++c) {
+            const int cb = cb0 + c;
+            double ai[2], dm[2], sp[2];
+#pragma unroll
+            for (int h = 0; h < 2; ++h) {
+                ai[h] = yi[c][h];
+                dm[h] = yr[c][h] - yi[c][h];
+                sp[h] = yr[c][h] + yi[c][h];
+            }
+#pragma unroll
+            for (int p = cb; p <= cb + 8; ++p) {
+                double k1[2] = {0.0, 0.0};
+#pragma unroll
+                for (int h = 0; h < 2; ++h) {
+                    c128 v = cmake(0.0, 0.0);
+                    double qv = 0.0;
+                    if ((p != cb || g >= 2 * t + h) && (p != cb + 8 || g < 2 * t + h)) {
+                        v = Vs[(8 * p + g) + (8 * cb + 2 * t + h) * BT_LDV];
+                        qv = Qs[(8 * p + g) + (8 * cb + 2 * t + h) * BT_LDV];
+                    }
+                    dmma_p(k1, ai[h], qv);
+                    dmma_p(zr[p], dm[h], v.x);
+                    dmma_p(zi[p], sp[h], v.y);
+                }
+                zr[p][0] += k1[0]; zr[p][1] += k1[1];
+                zi[p][0] += k1[0]; zi[p][1] += k1[1];
+            }
+        }
+        } else {
 #if BT_GAUSS2
         // Three real products per complex multiply-add (Gauss): with y = ar + i ai and v = vx + i vy,
         //   k1 = ar (vx + vy),  k2 = (ai - ar) vx,  k3 = (ar + ai) vy;   Re(y v) = k1 - k3,  Im(y v) = k1 + k2.
@@ -377,6 +434,7 @@ __device__ __forceinline__ void bt_apply_step(const c128* __restrict__ Vs, const
             }
         }
 #endif
+        }
         if (tail) {
             // rows beyond the matrix are virtual: keep them zero (stale V rows may have touched them)
 #pragma unroll
@@ -402,13 +460,16 @@ __global__ void __launch_bounds__(BT_NT, 1) bt_sweep_kernel(const BtSweepArgs a)
     constexpr int BT_STAGES = bt_stages(GS), BT_TSZ = bt_tsz(GS);
     c128* Tring = Vring + (size_t)BT_STAGES * BT_VS;
     c128* Zstage = Tring + (size_t)BT_STAGES * BT_TSZ;
-    BtHeader* hdr = reinterpret_cast<BtHeader*>(Zstage + (size_t)BT_CWARPS * BT_ZS);
+    double* Qring = reinterpret_cast<double*>(Zstage + (size_t)BT_CWARPS * BT_ZS);
+    BtHeader* hdr = reinterpret_cast<BtHeader*>(Qring + (bt_qplane(GS) ? (size_t)BT_STAGES * BT_VS : 0));
     uint64_t* full = reinterpret_cast<uint64_t*>(hdr + BT_STAGES);
     uint64_t* empty = full + BT_STAGES;
     uint64_t* zfull = empty + BT_STAGES;          // one per warp
 
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
     for (int idx = tid; idx < BT_STAGES * (BT_VS + BT_TSZ) + BT_CWARPS * BT_ZS; idx += BT_NT) Vring[idx] = cmake(0.0, 0.0);
+    if (bt_qplane(GS))
+        for (int idx = tid; idx < BT_STAGES * BT_VS; idx += BT_NT) Qring[idx] = 0.0;
     if (tid == 0) {
         for (int s = 0; s < BT_STAGES; ++s) { mbar_init(&full[s], 1); mbar_init(&empty[s], BT_CWARPS); }
         for (int w = 0; w < BT_CWARPS; ++w) mbar_init(&zfull[w], 1);
@@ -460,11 +521,13 @@ __global__ void __launch_bounds__(BT_NT, 1) bt_sweep_kernel(const BtSweepArgs a)
                 hh.nk_pred = (pr.pass + 1 < a.npass) ? (N - 1 - (pr.pass + 1) * BT_P + BT_B - 1) / BT_B : 0;
                 hh.pad0 = hh.pad1 = 0;
                 hdr[slot] = hh;
-                mbar_arrive_expect_tx(&full[slot], (uint32_t)((BT_VS + BT_TSZ) * sizeof(c128)));
+                mbar_arrive_expect_tx(&full[slot], (uint32_t)((BT_VS + BT_TSZ) * sizeof(c128) + (bt_qplane(GS) ? BT_VS * sizeof(double) : 0)));
                 // the 32 reflectors of (pass, k) are one contiguous, zero-padded 32 KB tile; -T is 32 (GS+1) elements
                 const int64_t stage = a.pass_off[pr.pass] + k;
                 bulk_g2s(Vring + (size_t)slot * BT_VS, a.V2 + stage * BT_VS, BT_VS * sizeof(c128), &full[slot]);
                 bulk_g2s(Tring + (size_t)slot * BT_TSZ, a.Tneg + stage * BT_TS, BT_TSZ * sizeof(c128), &full[slot]);
+                if (bt_qplane(GS))
+                    bulk_g2s(Qring + (size_t)slot * BT_VS, a.V2q + stage * BT_VS, BT_VS * sizeof(double), &full[slot]);
             }
         }
         ++pr.it;
@@ -515,9 +578,10 @@ __global__ void __launch_bounds__(BT_NT, 1) bt_sweep_kernel(const BtSweepArgs a)
                 }
         }
         const c128* Vs = Vring + (size_t)slot * BT_VS;
+        const double* Qs = Qring + (bt_qplane(GS) ? (size_t)slot * BT_VS : 0);
         const c128* Ts = Tring + (size_t)slot * BT_TSZ;
         constexpr int NSUB = BT_P / GS;
-        bt_apply_step<GS, NSUB - 1, NSUB - 1>(Vs, Ts, zr, zi, g, t, nrows < BT_WR, nrows);
+        bt_apply_step<GS, NSUB - 1, NSUB - 1>(Vs, Qs, Ts, zr, zi, g, t, nrows < BT_WR, nrows);
         // ---- prefetch the 64 rows that enter the window after this step: one 1-D bulk copy per column into
         //      this warp's staging tile (no registers, no LSU queue entries held across the step).  They are
         //      finalised by step k+1 of the predecessor.
@@ -538,9 +602,9 @@ __global__ void __launch_bounds__(BT_NT, 1) bt_sweep_kernel(const BtSweepArgs a)
                 bulk_g2s(Zs + lane * BT_LDZ, a.Z + (int64_t)mycol * a.ldz + R0 + BT_WR, (uint32_t)nin * (uint32_t)sizeof(c128),
                          &zfull[warp]);
         }
-        if constexpr (NSUB > 2) bt_apply_step<GS, (NSUB > 2 ? NSUB - 2 : 0), (NSUB > 2 ? 1 : 0)>(Vs, Ts, zr, zi, g, t, nrows < BT_WR, nrows);
+        if constexpr (NSUB > 2) bt_apply_step<GS, (NSUB > 2 ? NSUB - 2 : 0), (NSUB > 2 ? 1 : 0)>(Vs, Qs, Ts, zr, zi, g, t, nrows < BT_WR, nrows);
         if (warp == 0) produce();                 // stage it + STAGES - 1
-        if constexpr (NSUB > 1) bt_apply_step<GS, 0, 0>(Vs, Ts, zr, zi, g, t, nrows < BT_WR, nrows);
+        if constexpr (NSUB > 1) bt_apply_step<GS, 0, 0>(Vs, Qs, Ts, zr, zi, g, t, nrows < BT_WR, nrows);
         __syncwarp();
         if (lane == 0) mbar_arrive(&empty[slot]);
         if (last) {
@@ -662,6 +726,14 @@ int phase_backtransform_band(eigh_handle_s* h, const double* Qt, int64_t ldq, c1
                                                                            kmax, N, gs, pass_off, Tneg);
     h->launches += 2;
     BtSweepArgs a;
+    a.V2q = nullptr;
+    if (bt_qplane(gs)) {
+        const int64_t nel = v2_total_stages(N) * BT_VS;
+        double* V2q = ws_ptr<double>(h, pl.btQ);
+        bt_vq_kernel<<<(unsigned)std::min<int64_t>(ceil_div(nel, 256), 148 * 32), 256, 0, s>>>(ws_ptr<c128>(h, pl.V2), V2q, nel);
+        ++h->launches;
+        a.V2q = V2q;
+    }
     a.Z = Z; a.ldz = ldz; a.N = N; a.nev = nev; a.V2 = ws_ptr<c128>(h, pl.V2); a.Tneg = Tneg; a.pass_off = pass_off;
     a.npass = npass; a.nslabs = nslabs; a.unit_counter = counter; a.prog = prog;
     a.chain = h->bt_chain > 0 ? h->bt_chain : 1;      // chains of 2-4 passes cut the HBM traffic of Z but measure 0.4-1.6 % slower

@@ -27,6 +27,7 @@ struct WsPlan {
     size_t dc;                                 // D&C arena
     size_t dc_bytes;
     size_t Qt;                                 // D&C result N x nev real (lives inside dc arena)
+    size_t btQ;                                // S4a: q = Re v - Im v of the stage-2 reflectors (after btT when the dead D&C buffers hold both)
     size_t btT;                                // S4a: -T factors of all (pass, k) steps (aliases the dead D&C Q buffers)
     size_t bt;                                 // back-transform scratch (S4b's Y, S4a's counters)
     size_t bt_bytes;
