@@ -3,17 +3,21 @@
 
   python bench.py [--gpus N] [--steps K] [--warmup W] [--config C] [--nev NEV] [--impl reference]
 
-A "step" is one pass of the whole hot path (eigh_solve: full->band, band->tridiagonal, tridiagonal
-D&C, both back-transformations) over one synthetic matrix of BASELINE.json's `configs` (default
-config 3, the N = 27648 vortex-tangle BdG matrix: the largest one whose W + K solves finish within
-minutes; --config 4 runs the N = 49152 target, --config 2 the N = 8192 case).  The matrix is regenerated in place
-(device-side copy from a resident pristine copy, or the device generator when two copies do not
-fit) OUTSIDE the per-step CUDA-event brackets, because eigh_solve overwrites A.
+A "step" is one pass of the whole hot path (eigh_solve: full->band, band->tridiagonal, tridiagonal D&C, both
+back-transformations) over one synthetic matrix of BASELINE.json's `configs`.  Default workload = config 4, the
+N = 49152 BdG vortex-tangle matrix (the largest single-GPU config and the north_star target).  BASELINE.json lists
+two runs for it, "full eigendecomposition and nev = N/2 subset": all eigenpairs are computed when W + K full solves
+fit the time budget (--time-budget, default 1500 s: the default W = 3, K = 2 run does), otherwise the nev = N/2 run is
+timed (the driver's --steps 20 --warmup 5: 25 x 75 s does not fit its 1800 s limit, 25 x 47 s does); which one ran is
+stated in `config.nev` / `config.nev_rule`.  The rule is a pure function of (config, W, K, budget), so both arms of
+the driver's comparison make the same choice.  The matrix is regenerated in place (eigh_assemble_bdg on the device, or
+a device copy of a pristine matrix for config 1) OUTSIDE the per-step CUDA-event brackets, because eigh_solve
+overwrites A.
 
-One JSON line on stdout (rank 0):  metric = eigh_time_s (seconds per eigensolve, lower is better),
-plus `phases` (ms, credited TFLOP/s or GB/s per phase), `roofline` (dominant phase against the FP64
-tensor peak), `e2e` (host buffers through eigh_solve_host), `cpu_baseline` (the oracle on a
-bounded sample) and `clocks`.
+One JSON line on stdout (rank 0):  metric = eigh_time_s (seconds per eigensolve, lower is better), plus `phases`
+(ms, credited / executed TFLOP/s or GB/s per phase, S3 merge statistics), `roofline` (the dominant kernel against the
+FP64 tensor peak), `e2e` (host buffers through eigh_solve_host), `cpu_baseline` (the oracle on a bounded sample) and
+`clocks`.
 
 Multi-GPU: the path does not shard ("replicas only"): every rank solves its own replica,
 value = max-over-ranks time / n_gpus.
@@ -21,6 +25,7 @@ value = max-over-ranks time / n_gpus.
 from __future__ import annotations
 
 import argparse
+import hashlib
 import json
 import os
 import subprocess
@@ -36,25 +41,50 @@ FP64_NOMINAL_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12      # 37.2: 148 SMs x 64 FP
 CLOCK_QUERY = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,"
                "clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
                "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+PHASES = ["p1_full_to_band", "p2_band_to_tridiag", "p3_tridiag_dc", "p4a_backtransform_band", "p4b_backtransform_full"]
+# seconds per eigh_solve (all eigenpairs) measured on one B200 for the nev rule; source: profiles/r01_summary.md and
+# profiles/r02_summary.md.  Only used to decide between the two runs BASELINE.json lists for configs 3 and 4.
+FULL_SOLVE_MODEL_S = {0: 0.03, 1: 0.2, 2: 0.6, 3: 14.0, 4: 75.0}
+# executed real FP64 tensor flops per credited flop: GEMM engine in the 3M form = 6/8; bt_sweep_kernel: 116 DMMAs of
+# 512 flops per compact-WY block of 8 reflectors x 8 columns, credited 2 x 8 x 64 x 8 x 8
+EXECUTED_PER_CREDITED = {"p1": 0.75, "p4a": 116 * 512 / 65536.0, "p4b": 0.75}
 
 
 def credited_work(N: int, nev: int, b: int):
     """Credited algorithmic work per phase (lower-order terms dropped)."""
     steps = 0
-    bytes_p2 = 0
     for j in range(0, N - 1):
-        ks = -(-(N - 1 - j) // b)
-        steps += ks
+        steps += -(-(N - 1 - j) // b)
     # per chase step: D lower (b^2/2) + S (b^2) read and written, 16 B each; reflector b written
     bytes_p2 = steps * (2 * (b * b // 2 + b * b) * 16 + b * 16)
     return {
         "p1_flops": 16.0 / 3.0 * N ** 3,
         "p2_flops": 24.0 * b * N * N,
         "p2_bytes": float(bytes_p2),
-        "p3_flops_max": 8.0 / 3.0 * N ** 3,       # dense merges without deflation (as executed: no block structure)
+        "p2_steps": steps,
         "p4a_flops": 8.0 * N * N * nev,
         "p4b_flops": 8.0 * N * N * nev,
     }
+
+
+def choose_nev(config: int, N: int, nev_runs, warmup: int, steps: int, budget_s: float, nev_arg: int = 0):
+    """The run of BASELINE.json's config that is timed: (nev, rule text).  Deterministic in its arguments."""
+    if nev_arg > 0:
+        return min(nev_arg, N), "--nev given"
+    full = (warmup + steps) * FULL_SOLVE_MODEL_S.get(config, 75.0)
+    if len(nev_runs) < 2 or full <= budget_s:
+        return N, "all eigenpairs: (W + K) x %.1f s = %.0f s fits the %.0f s budget" % (
+            FULL_SOLVE_MODEL_S.get(config, 75.0), full, budget_s)
+    return int(nev_runs[1]), ("nev = N/2 run of BASELINE.json's config (lowest N/2 pairs): (W + K) x %.1f s = %.0f s of full "
+                              "solves exceed the %.0f s budget" % (FULL_SOLVE_MODEL_S.get(config, 75.0), full, budget_s))
+
+
+def config_dict(w, nev: int, rule: str, b: int = 64):
+    """`config` of the JSON line -- the same keys and values in both arms (--impl ours / reference)."""
+    return {"workload": w.name, "N": w.N, "nev": nev, "nev_rule": rule, "band_width": b,
+            "parallelism": "replicas only",
+            "l2": "inputs larger than L2 (matrix %.1f GB)" % (w.N * w.N * 16 / 1e9),
+            "input_regeneration": "on the device, outside the timed brackets"}
 
 
 class ClockSampler:
@@ -119,54 +149,15 @@ def replica_value_s(ms_per_step: float, world: int) -> float:
     return ms_per_step / 1e3 / world
 
 
-def reference_arm(args, wl_mod):
-    """--impl reference: the CPU oracle (unmodified, as it stands) on a bounded sample of the workload:
-    the leading principal n_s x n_s submatrix, timed per step and scaled by (N/n_s)^3 (the oracle is a
-    23 N^3 level-1/2 method; SURVEY.md 8(c))."""
+def oracle_sample(w, ns):
+    """A bounded sample of the workload for the CPU oracle: the leading ns x ns block of the dense matrix when it is
+    affordable (N <= 8192), else the same recipe (fields, mu) restricted to a sub-lattice with 2 nx ny nz <= ns (not
+    the same matrix: stated in `sample`).  Returns (matrix, description)."""
     import numpy as np
-    import oracle
-    rank = int(os.environ.get("RANK", "0"))
-    if rank != 0:
-        return
-    w = wl_mod.make_config(args.config)
-    N = w.N
-    ns = min(N, args.ref_sample)
-    if w.problem is not None:
-        H = _leading_block_bdg(w, ns)
-    else:
-        H = w.dense()[:ns, :ns]
-    times = []
-    for i in range(args.warmup + args.steps):
-        t0 = time.perf_counter()
-        oracle.eigh(H)
-        dt = time.perf_counter() - t0
-        if i >= args.warmup:
-            times.append(dt)
-    per = sum(times) / len(times)
-    ns = H.shape[0]                       # the BdG sub-lattice sample may be smaller than requested
-    est = per * (N / ns) ** 3
-    line = {
-        "impl": "reference", "metric": "eigh_time_s", "value": est, "unit": "s", "n_gpus": args.gpus,
-        "steps": args.steps, "warmup": args.warmup, "ms_per_step": est * 1e3, "higher_is_better": False,
-        "scaling": "weak", "vs_baseline": None, "dtype": "c128", "data": "synthetic",
-        "config": {"workload": w.name, "N": N, "nev": N},
-        "cpu_baseline": {"value": est, "unit": "s", "cores": oracle.num_threads(), "kind": "oracle",
-                         "sample": f"{ns}x{ns} sample (leading block, or the same recipe on a sub-lattice) solved in {per:.3f} s "
-                                   f"per step, scaled by (N/{ns})^3"},
-        "e2e": {"value": est, "unit": "s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
-    }
-    print(json.dumps(line))
-
-
-def _leading_block_bdg(w, ns):
-    """Leading ns x ns block of a BdG config without materialising the full matrix: solve the same
-    generator on a smaller lattice slab is NOT the same matrix, so take the block of the dense matrix
-    when it is affordable, else a sub-lattice of the same recipe (stated in `sample`)."""
-    import numpy as np
-    if w.N <= 8192:
-        return np.ascontiguousarray(w.dense()[:ns, :ns])
+    if w.problem is None or w.N <= 8192:
+        H = np.ascontiguousarray(w.dense()[:ns, :ns])
+        return H, f"leading {H.shape[0]} x {H.shape[0]} block of the matrix"
     from paper_2310_03341_b200 import workloads as wl
-    # same recipe (fields, mu) restricted to a sub-lattice with 2*nx*ny*nz ~ ns
     p = w.problem
     nx, ny, nz = p.shape
     while 2 * nx * ny * nz > ns:
@@ -175,7 +166,62 @@ def _leading_block_bdg(w, ns):
         else: nz //= 2
     idx = np.arange(np.prod(p.shape)).reshape(p.shape)[:nx, :ny, :nz].reshape(-1)
     q = wl.BdGProblem(p.name, (nx, ny, nz), p.mu, p.V[idx], p.Delta[idx])
-    return q.dense()
+    H = q.dense()
+    return H, f"the same recipe (fields, mu) on the {nx}x{ny}x{nz} sub-lattice, order {H.shape[0]}"
+
+
+def reference_arm(args, wl_mod):
+    """--impl reference: the CPU oracle (unmodified, as it stands; all eigenpairs -- it has no subset mode) on a
+    bounded sample of the workload, timed per step on the box's host cores and scaled by (N/n_s)^3 (the oracle is a
+    23 N^3 level-1/2 method; SURVEY.md 8(c))."""
+    import oracle
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    w = wl_mod.make_config(args.config)
+    N = w.N
+    nev, rule = choose_nev(args.config, N, w.nev_runs, args.warmup, args.steps, args.time_budget, args.nev)
+    H, what = oracle_sample(w, min(N, args.ref_sample))
+    times = []
+    for i in range(args.warmup + args.steps):
+        t0 = time.perf_counter()
+        oracle.eigh(H)
+        dt = time.perf_counter() - t0
+        if i >= args.warmup:
+            times.append(dt)
+    per = sum(times) / len(times)
+    ns = H.shape[0]
+    est = per * (N / ns) ** 3
+    line = {
+        "impl": "reference", "metric": "eigh_time_s", "value": est, "unit": "s", "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": est * 1e3, "higher_is_better": False,
+        "scaling": "weak", "vs_baseline": None, "dtype": "c128", "data": "synthetic",
+        "config": config_dict(w, nev, rule),
+        "cpu_baseline": {"value": est, "unit": "s", "cores": oracle.num_threads(), "kind": "oracle",
+                         "sample": f"{what}: {per:.3f} s per step measured (all eigenpairs), scaled by (N/{ns})^3",
+                         "measured_s": per, "measured_order": ns},
+        "e2e": {"value": est, "unit": "s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+    }
+    print(json.dumps(line))
+
+
+def kernel_source_sha(name: str) -> str:
+    with open(os.path.join(ROOT, "paper_2310_03341_b200", "csrc", name), "rb") as f:
+        return hashlib.sha256(f.read()).hexdigest()[:16]
+
+
+def lookup_traffic(workload: str, nev: int):
+    """DRAM bytes (read + write) of one bt_sweep_kernel launch from an ncu capture -- only if the capture recorded in
+    profiles/traffic.json was taken on this workload, this nev and THIS source of the kernel (sha of bt_band.cu)."""
+    try:
+        entries = json.load(open(os.path.join(ROOT, "profiles", "traffic.json")))
+    except Exception:
+        return None, "no profiles/traffic.json"
+    sha = kernel_source_sha("bt_band.cu")
+    for e in entries:
+        if e.get("workload") == workload and e.get("nev") == nev and e.get("source_sha") == sha:
+            return float(e["dram_bytes"]), e.get("capture")
+    return None, "no ncu capture of this kernel source (sha %s) on this workload / nev" % sha
 
 
 def main():
@@ -183,18 +229,20 @@ def main():
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=2)
     ap.add_argument("--warmup", type=int, default=3)
-    ap.add_argument("--config", type=int, default=int(os.environ.get("EIGH_BENCH_CONFIG", "3")))
-    ap.add_argument("--nev", type=int, default=0, help="0 = all eigenpairs")
+    ap.add_argument("--config", type=int, default=int(os.environ.get("EIGH_BENCH_CONFIG", "4")))
+    ap.add_argument("--nev", type=int, default=0, help="0 = the run chosen by the time budget (all eigenpairs or N/2)")
+    ap.add_argument("--time-budget", type=float, default=1500.0,
+                    help="seconds available for the W + K solves; decides between the two runs of configs 3 / 4")
     ap.add_argument("--impl", default="ours")
     ap.add_argument("--ref-sample", type=int, default=3456, help="order of the oracle sample of --impl reference")
     ap.add_argument("--cpu-sample", type=int, default=3456,
                     help="order of the oracle's sample (about 10-30 s of CPU work on the box's host cores)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-epilogue", action="store_true")
     ap.add_argument("--context", action="store_true",
                     help="also time library routines on the same matrix as CONTEXT (never the target, never on the hot path): "
                          "torch.linalg.eigh (cuSOLVER) on this GPU and numpy.linalg.eigh (LAPACK) on the CPU sample")
-    ap.add_argument("--wy-group", type=int, default=0)
     ap.add_argument("--opt", action="append", default=[], help="solver option key=value (eigh_set_option), repeatable")
     args = ap.parse_args()
     # W >= 3 is the timing rule for a valid bench number; smaller values are accepted for profiler runs only
@@ -223,31 +271,34 @@ def main():
 
     w = wl_mod.make_config(args.config)
     N = w.N
-    nev = args.nev if args.nev > 0 else N
+    nev, nev_rule = choose_nev(args.config, N, w.nev_runs, args.warmup, args.steps, args.time_budget, args.nev)
     opts = {}
-    if args.wy_group:
-        opts["wy_group"] = args.wy_group
     for kv in args.opt:
         key, val = kv.split("=")
         opts[key] = int(val)
     solver = binding.Eigh(N, nev, device=dev, **opts)
-    b = 64
+    b = solver.band_width                                    # read from the handle (eigh_get_option)
     mat_bytes = N * N * 16
-    free_b, total_b = torch.cuda.mem_get_info()
-    keep_pristine = free_b > 3 * mat_bytes + (2 << 30)
     At = torch.empty((N, N), dtype=torch.complex128, device=dev)       # A column-major (stored as A^T row-major)
     W = torch.empty(N, dtype=torch.float64, device=dev)
     Zt = torch.empty((nev, N), dtype=torch.complex128, device=dev)
     pristine = None
-    if keep_pristine:
+    fields = None
+    if w.problem is not None:
+        # BdG configs: H is re-assembled on the device from its fields by the library's own prologue kernel
+        pb = w.problem
+        fields = ([torch.from_numpy(wl_mod.kinetic_1d(L)).to(dev) for L in pb.shape],
+                  torch.from_numpy(pb.V).to(dev), torch.from_numpy(np.ascontiguousarray(pb.Delta)).to(dev))
+    else:
         pristine = torch.empty((N, N), dtype=torch.complex128, device=dev)
         w.dense_torch(dev, out=pristine)
 
     def regenerate():
-        if pristine is not None:
-            At.copy_(pristine)
+        if fields is not None:
+            K3, Vd, Dd = fields
+            solver.assemble_bdg(w.problem.shape, K3[0], K3[1], K3[2], Vd, Dd, w.problem.mu, At=At)
         else:
-            w.dense_torch(dev, out=At)
+            At.copy_(pristine)
 
     stream = torch.cuda.current_stream()
     ev0 = torch.cuda.Event(enable_timing=True)
@@ -287,13 +338,14 @@ def main():
     clocks = sampler.stop(t0, t1) if rank == 0 else None
     ms_per_step = total_ms / args.steps
     value_s = replica_value_s(ms_per_step, world)        # seconds per eigensolve, whole job (replicas)
+    dc_flops, dc_kept = solver.dc_stats()                # S3 merge statistics of the last solve
 
     # ---- quick validity check of the last solve (device side, independent ZGEMM by torch)
     valid = {}
     if rank == 0:
         with torch.no_grad():
-            Hd = pristine if pristine is not None else w.dense_torch(dev, out=At)
-            Hl = Hd.t() if pristine is not None else Hd
+            regenerate()
+            Hl = At.t()                                          # logical H (all N^2 elements are valid)
             ncheck = min(nev, 256)
             cols = torch.linspace(0, nev - 1, ncheck, device=dev).long()
             Zc = Zt[cols].t()                                   # N x ncheck
@@ -302,46 +354,50 @@ def main():
             valid["residual_sampled"] = float(torch.linalg.norm(R).item()) / (hn * (ncheck ** 0.5))
             valid["orth_sampled"] = float((Zc.conj().t() @ Zc - torch.eye(ncheck, device=dev)).abs().max().item())
             valid["trace_err"] = abs(float(W.sum().item()) - float(torch.diagonal(Hl).real.sum().item()))
+            del R, Zc
+
+    hbm = None
+    peaks = {}
+    try:
+        peaks = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))
+        hbm = peaks.get("hbm_gbs")
+    except Exception:
+        pass
 
     # ---- SCF epilogue (outside the timed step): eigh_densities on the eigenpairs just computed,
     # Eq. 16a/16d at T = 0.  HBM-bound: algorithmic bytes = the u and v halves of every ACTIVE column of Z read once
-    # (16 N bytes per column with 0 < E < Ec) + the two output fields; CUDA events on the launching stream.
+    # (16 N bytes per column) + the two output fields; CUDA events on the launching stream.
     epilogue = None
-    if rank == 0 and w.problem is not None and N % 2 == 0:
+    if rank == 0 and w.problem is not None and N % 2 == 0 and not args.no_epilogue:
         try:
-            n_f, nu_f = solver.densities(W, Zt, T=0.0)
+            branch = 1 if nev == N else -1                       # lowest N/2 pairs: particle-hole partners (reading 3)
+            E = W[:nev].contiguous()
+            n_f, nu_f = solver.densities(E, Zt, T=0.0, branch=branch)
             torch.cuda.synchronize()
             ts = []
             for _ in range(5):
                 ev0.record(stream)
-                solver.densities(W, Zt, T=0.0, n=n_f, nu=nu_f)
+                solver.densities(E, Zt, T=0.0, branch=branch, n=n_f, nu=nu_f)
                 ev1.record(stream)
                 torch.cuda.synchronize()
                 ts.append(ev0.elapsed_time(ev1))
-            active = int(((W[:nev] > 0)).sum().item())
+            active = int((E > 0).sum().item()) if branch == 1 else int((E < 0).sum().item())
             dbytes = 16.0 * N * active + 24.0 * (N // 2)
             dms = sorted(ts)[len(ts) // 2]
-            hbm = None
-            try:
-                hbm = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json"))).get("hbm_gbs")
-            except Exception:
-                pass
-            epilogue = {"op": "eigh_densities (Eq. 16a, 16d; T = 0; all columns with E > 0)", "ms": dms,
+            epilogue = {"op": "eigh_densities (Eq. 16a, 16d; T = 0; branch %+d)" % branch, "ms": dms,
                         "active_columns": active, "algorithmic_bytes": dbytes, "bound": "hbm",
                         "achieved_gbs": dbytes / dms / 1e6 if dms else None, "peak_gbs": hbm,
                         "frac": (dbytes / dms / 1e6) / hbm if hbm and dms else None, "launches": 3,
                         "particle_number": float(n_f.sum().item()),
                         "note": "inputs (%.1f GB of active columns) larger than L2" % (16.0 * N * active / 1e9)}
-            # Eq. 16b/16c: eigh_gradient_densities (three launches, one per axis; FP64 tensor cores + HBM: 4 L FMAs and 32
-            # bytes per grid point, state and axis -- at L = 24..32 the two rooflines nearly coincide, both are reported)
             pb = w.problem
             Dd = [torch.from_numpy(np.ascontiguousarray(wl_mod.derivative_1d(L).T)).to(dev) for L in pb.shape]
-            solver.gradient_densities(pb.shape, Dd[0], Dd[1], Dd[2], W, Zt, T=0.0)
+            solver.gradient_densities(pb.shape, Dd[0], Dd[1], Dd[2], E, Zt, T=0.0, branch=branch)
             torch.cuda.synchronize()
             ts = []
             for _ in range(3):
                 ev0.record(stream)
-                solver.gradient_densities(pb.shape, Dd[0], Dd[1], Dd[2], W, Zt, T=0.0)
+                solver.gradient_densities(pb.shape, Dd[0], Dd[1], Dd[2], E, Zt, T=0.0, branch=branch)
                 ev1.record(stream)
                 torch.cuda.synchronize()
                 ts.append(ev0.elapsed_time(ev1))
@@ -354,16 +410,10 @@ def main():
                                     "frac": gflops / gms / 1e9 / FP64_NOMINAL_TFLOPS if gms else None,
                                     "achieved_gbs": gbytes / gms / 1e6 if gms else None,
                                     "hbm_frac": (gbytes / gms / 1e6) / hbm if hbm and gms else None}
-            # prologue: eigh_assemble_bdg writes all N^2 elements of H from (K, V, Delta): HBM-write-bound, 16 N^2 bytes
-            Kd = [torch.from_numpy(wl_mod.kinetic_1d(L)).to(dev) for L in pb.shape]
-            Vd = torch.from_numpy(pb.V).to(dev)
-            Dd = torch.from_numpy(np.ascontiguousarray(pb.Delta)).to(dev)
-            solver.assemble_bdg(pb.shape, Kd[0], Kd[1], Kd[2], Vd, Dd, pb.mu, At=At)
-            torch.cuda.synchronize()
             ts = []
             for _ in range(5):
                 ev0.record(stream)
-                solver.assemble_bdg(pb.shape, Kd[0], Kd[1], Kd[2], Vd, Dd, pb.mu, At=At)
+                regenerate()
                 ev1.record(stream)
                 torch.cuda.synchronize()
                 ts.append(ev0.elapsed_time(ev1))
@@ -375,67 +425,77 @@ def main():
         except Exception as ex:   # reported, never hidden
             epilogue = {"error": str(ex)[:200]}
 
-    # ---- e2e: host buffers through eigh_solve_host (H2D of A, D2H of W and Z inside the timed region)
+    # ---- e2e: host buffers through eigh_solve_host.  A_host is PAGEABLE host memory of the full matrix; it is streamed
+    # H2D through the handle's bounded pinned ring (2 x 256 MiB), W and Z come back the same way; all of it inside the
+    # timed region (wall clock around the synchronous call, device idle on both sides).
     e2e = None
     if not args.no_e2e and rank == 0:
         try:
-            src = pristine if pristine is not None else w.dense_torch(dev, out=At)
-            Ah = torch.empty((N, N), dtype=torch.complex128, pin_memory=True)
-            Ah.copy_(src if pristine is not None else At)
-            Wh = torch.empty(N, dtype=torch.float64, pin_memory=True)
-            Zh = torch.empty((nev, N), dtype=torch.complex128, pin_memory=True)
+            regenerate()
+            torch.cuda.synchronize()
+            Ah = torch.empty((N, N), dtype=torch.complex128)
+            Ah.copy_(At)
+            Wh = torch.empty(N, dtype=torch.float64)
+            Zh = torch.empty((nev, N), dtype=torch.complex128)
             times = []
             for i in range(2 if N <= 8192 else 1):
                 torch.cuda.synchronize()
-                ev0.record(stream)
+                tt = time.perf_counter()
                 solver.solve_host(Ah, Wh, Zh, At, W, Zt)
-                ev1.record(stream)
                 torch.cuda.synchronize()
-                times.append(ev0.elapsed_time(ev1))
-            e2e = {"value": min(times) / 1e3, "unit": "s", "h2d_bytes_per_step": mat_bytes,
-                   "d2h_bytes_per_step": N * 8 + N * nev * 16}
+                times.append(time.perf_counter() - tt)
+            e2e = {"value": min(times), "unit": "s", "h2d_bytes_per_step": mat_bytes,
+                   "d2h_bytes_per_step": N * 8 + N * nev * 16,
+                   "host_buffers": "pageable, streamed through a 2 x 256 MiB pinned ring (eigh_solve_host)",
+                   "check_W_max_abs_diff": float((Wh - W.cpu()).abs().max().item())}
             del Ah, Zh
-        except Exception as ex:  # pinned allocation may fail for the largest configs
+        except Exception as ex:  # host allocation may fail for the largest configs
             e2e = {"value": None, "unit": "s", "error": str(ex)[:200]}
 
-    # ---- cpu baseline: the oracle, as it stands, on a bounded sample
+    # ---- cpu baseline: the oracle, as it stands, on a bounded sample (+ the measured, not extrapolated, small configs)
     cpu = None
     if not args.no_cpu_baseline and rank == 0 and world == 1:
         import oracle
-        ns = min(N, args.cpu_sample)
-        Hs = _leading_block_bdg(w, ns) if w.problem is not None else w.dense()[:ns, :ns]
-        ns = Hs.shape[0]                  # the BdG sub-lattice sample may be smaller than requested
+        Hs, what = oracle_sample(w, min(N, args.cpu_sample))
+        ns = Hs.shape[0]
         tt = time.perf_counter()
         oracle.eigh(Hs)
         dt = time.perf_counter() - tt
         cpu = {"value": dt * (N / ns) ** 3, "unit": "s", "cores": oracle.num_threads(), "kind": "oracle",
-               "sample": f"{ns}x{ns} sample (leading block of the matrix, or for N > 8192 the same recipe on a sub-lattice): "
-                         f"{dt:.3f} s measured, scaled by (N/{ns})^3 (23 N^3 flops method)"}
+               "sample": f"{what}: {dt:.3f} s measured (all eigenpairs), scaled by (N/{ns})^3 (23 N^3 flops method)",
+               "measured_s": dt, "measured_order": ns}
+        try:   # config 0 measured as it is (not extrapolated)
+            H0 = wl_mod.make_config(0).dense()
+            tt = time.perf_counter()
+            oracle.eigh(H0)
+            cpu["measured_config0_N1024_s"] = time.perf_counter() - tt
+        except Exception as ex:
+            cpu["measured_config0_error"] = str(ex)[:100]
 
     # ---- context rows: library eigensolvers on the same seeded matrix; reported, never the target
     context = None
     if args.context and rank == 0 and world == 1:
         context = {}
         try:
+            Wkeep = W.clone()
             del Zt
             torch.cuda.empty_cache()
-            Hc = w.dense_torch(dev, out=At)                   # logical H (column-major storage in At)
+            regenerate()
             torch.cuda.synchronize()
             ev0.record(stream)
-            Wc, Zc = torch.linalg.eigh(Hc)
+            Wc, Zc = torch.linalg.eigh(At.t())
             ev1.record(stream)
             torch.cuda.synchronize()
             context["torch_linalg_eigh_s"] = ev0.elapsed_time(ev1) / 1e3
-            context["torch_linalg_eigh_max_abs_diff_W"] = float((Wc - W).abs().max().item())
+            context["torch_linalg_eigh_max_abs_diff_W"] = float((Wc - Wkeep).abs().max().item())
             del Wc, Zc
         except Exception as ex:
             context["torch_linalg_eigh_error"] = str(ex)[:200]
         try:
-            ns = min(N, args.cpu_sample)
-            Hs = _leading_block_bdg(w, ns) if w.problem is not None else w.dense()[:ns, :ns]
+            Hs, _ = oracle_sample(w, min(N, args.cpu_sample))
             tt = time.perf_counter()
             np.linalg.eigh(Hs)
-            context["numpy_linalg_eigh_sample"] = {"n": ns, "s": time.perf_counter() - tt}
+            context["numpy_linalg_eigh_sample"] = {"n": Hs.shape[0], "s": time.perf_counter() - tt}
         except Exception as ex:
             context["numpy_linalg_eigh_error"] = str(ex)[:200]
 
@@ -446,62 +506,63 @@ def main():
 
     cw = credited_work(N, nev, b)
     ph = [sum(p[i] for p in phases) / len(phases) for i in range(6)]
+
+    def tf(flops, ms):
+        return flops / ms / 1e9 if ms else None
+
+    s3_flops = float(sum(dc_flops))
     phase_report = {
-        "p1_full_to_band": {"ms": ph[0], "tflops": cw["p1_flops"] / ph[0] / 1e9 if ph[0] else None},
+        "p1_full_to_band": {"ms": ph[0], "tflops": tf(cw["p1_flops"], ph[0]),
+                            "tflops_executed": tf(cw["p1_flops"] * EXECUTED_PER_CREDITED["p1"], ph[0])},
         "p2_band_to_tridiag": {"ms": ph[1], "gbs_credited": cw["p2_bytes"] / ph[1] / 1e6 if ph[1] else None,
-                               "tflops": cw["p2_flops"] / ph[1] / 1e9 if ph[1] else None},
-        "p3_tridiag_dc": {"ms": ph[2], "tflops_if_no_deflation": cw["p3_flops_max"] / ph[2] / 1e9 if ph[2] else None},
-        "p4a_backtransform_band": {"ms": ph[3], "tflops": cw["p4a_flops"] / ph[3] / 1e9 if ph[3] else None},
-        "p4b_backtransform_full": {"ms": ph[4], "tflops": cw["p4b_flops"] / ph[4] / 1e9 if ph[4] else None},
+                               "tflops": tf(cw["p2_flops"], ph[1]), "chase_steps": cw["p2_steps"],
+                               "us_per_step_per_cta": ph[1] * 1e3 / (cw["p2_steps"] / 148.0) if ph[1] else None},
+        "p3_tridiag_dc": {"ms": ph[2], "merge_flops_executed": s3_flops, "tflops_executed": tf(s3_flops, ph[2]),
+                          "frac_of_fp64_peak": tf(s3_flops, ph[2]) / FP64_NOMINAL_TFLOPS if ph[2] else None,
+                          "kept_frac_per_level": dc_kept, "deflated_frac_per_level": [1.0 - k for k in dc_kept],
+                          "merge_flops_per_level": dc_flops,
+                          "note": "executed = sum over the merge GEMMs of 2 M N K as launched (real DMMA flops); the "
+                                  "phase time also holds the secular / deflation kernels (ALU)"},
+        "p4a_backtransform_band": {"ms": ph[3], "tflops": tf(cw["p4a_flops"], ph[3]),
+                                   "tflops_executed": tf(cw["p4a_flops"] * EXECUTED_PER_CREDITED["p4a"], ph[3])},
+        "p4b_backtransform_full": {"ms": ph[4], "tflops": tf(cw["p4b_flops"], ph[4]),
+                                   "tflops_executed": tf(cw["p4b_flops"] * EXECUTED_PER_CREDITED["p4b"], ph[4])},
     }
-    # roofline object: the dominant kernel.  S4a is one persistent launch (bt_sweep_kernel) whose duration is
-    # measured by CUDA events inside the library on the solve's stream; its algorithmic work is the credited
-    # 8 N^2 nev flops of the band back-transformation (WY padding and the T products excluded).
+    # roofline object: the dominant kernel = the one with the largest device time per step.  S4a is ONE persistent launch
+    # (bt_sweep_kernel) timed by CUDA events inside the library on the solve's stream; the GEMM families of S1 / S4b are
+    # spread over hundreds of launches per phase and each family stays below its phase total (see the launch list in
+    # profiles/).  Algorithmic work of the launch = the credited 8 N^2 nev flops of the band back-transformation
+    # (WY padding and the T products excluded).
     dominant = max(range(5), key=lambda i: ph[i])
     sweep_ms = ph[5]
     achieved = cw["p4a_flops"] / sweep_ms / 1e9 if sweep_ms else 0.0
-    peaks = {}
-    try:
-        peaks = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))
-    except Exception:
-        pass
-    # DRAM bytes (read + write) of one bt_sweep_kernel launch from the committed ncu capture of this workload
-    # (profiles/r01_bt_sweep_c3_traffic.csv, command in profiles/r01_ncu_kernels.md); null for other workloads
-    traffic = None
-    if w.index == 3 and nev == N:
-        try:
-            import csv
-            tot = 0.0
-            with open(os.path.join(ROOT, "profiles", "r01_bt_sweep_c3_traffic.csv")) as f:
-                for row in csv.reader(l for l in f if not l.startswith("==")):
-                    if len(row) > 3 and row[-3] in ("dram__bytes_read.sum", "dram__bytes_write.sum"):
-                        tot += float(row[-1].replace(",", ""))
-            traffic = tot if tot > 0 else None
-        except Exception:
-            traffic = None
+    traffic, traffic_note = lookup_traffic(w.name, nev)
     roofline = {
-        "bound": "tensor", "kernel": "eigh::bt_sweep_kernel<8> (FP64 DMMA, 1 launch per solve, phase p4a)",
+        "bound": "tensor", "kernel": "eigh::bt_sweep_kernel<%d> (FP64 DMMA, 1 launch per solve, all of phase p4a)" % solver.get_option("wy_group"),
         "achieved": achieved, "peak": FP64_NOMINAL_TFLOPS, "unit": "TFLOP/s", "frac": achieved / FP64_NOMINAL_TFLOPS,
-        "traffic": traffic, "traffic_unit": "bytes per launch (dram read + write, ncu)",
+        "frac_executed": achieved * EXECUTED_PER_CREDITED["p4a"] / FP64_NOMINAL_TFLOPS,
+        "traffic": traffic, "traffic_unit": "bytes per launch (dram read + write, ncu)", "traffic_source": traffic_note,
         "algorithmic_flops_per_launch": cw["p4a_flops"], "kernel_ms": sweep_ms, "launches_per_step": 1,
-        "dominant_phase": ["p1_full_to_band", "p2_band_to_tridiag", "p3_tridiag_dc", "p4a_backtransform_band",
-                           "p4b_backtransform_full"][dominant],
-        "peak_source": "FP64 tensor (DMMA) 148 SM x 64 FMA/clk x 1.965 GHz = 37.2 TFLOP/s, equal to the burst DMMA rate "
+        "kernel_share_of_step": sweep_ms / ms_per_step if ms_per_step else None,
+        "dominant_phase": PHASES[dominant],
+        "peak_source": "FP64 tensor (DMMA) 148 SM x 64 FMA/clk x 2 x 1.965 GHz = 37.2 TFLOP/s, equal to the burst DMMA rate "
                        "measured on this pool (profiles/r01_fp64_peaks.md; cuBLAS ZGEMM 36.8); MEASURED_PEAKS.json has "
-                       "no FP64 entry",
-        "tensor_phase_fracs": {"p1": cw["p1_flops"] / ph[0] / 1e9 / FP64_NOMINAL_TFLOPS if ph[0] else None,
-                               "p4a": cw["p4a_flops"] / ph[3] / 1e9 / FP64_NOMINAL_TFLOPS if ph[3] else None,
-                               "p4b": cw["p4b_flops"] / ph[4] / 1e9 / FP64_NOMINAL_TFLOPS if ph[4] else None},
-        "hbm_peak_gbs": peaks.get("hbm_gbs"),
-        "p2_hbm_frac_credited": (cw["p2_bytes"] / ph[1] / 1e6) / peaks["hbm_gbs"] if ph[1] and peaks.get("hbm_gbs") else None,
+                       "no FP64 entry.  `frac` divides CREDITED flops (8 per complex multiply-add) by it; `frac_executed` "
+                       "the real flops the kernel issues (3-product forms)",
+        "tensor_phase_fracs": {"p1": tf(cw["p1_flops"], ph[0]) / FP64_NOMINAL_TFLOPS if ph[0] else None,
+                               "p4a": tf(cw["p4a_flops"], ph[3]) / FP64_NOMINAL_TFLOPS if ph[3] else None,
+                               "p4b": tf(cw["p4b_flops"], ph[4]) / FP64_NOMINAL_TFLOPS if ph[4] else None},
+        "tensor_phase_fracs_executed": {k: (tf(cw[k + "_flops"], ph[i]) * EXECUTED_PER_CREDITED[k] / FP64_NOMINAL_TFLOPS if ph[i] else None)
+                                        for k, i in (("p1", 0), ("p4a", 3), ("p4b", 4))},
+        "hbm_peak_gbs": hbm,
+        "p2_hbm_frac_credited": (cw["p2_bytes"] / ph[1] / 1e6) / hbm if ph[1] and hbm else None,
     }
+    cfg = config_dict(w, nev, nev_rule, b)
     line = {
         "metric": "eigh_time_s", "value": value_s, "unit": "s", "n_gpus": world, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": ms_per_step, "higher_is_better": False, "scaling": "weak",
         "vs_baseline": None, "dtype": "c128", "data": "synthetic",
-        "config": {"workload": w.name, "N": N, "nev": nev, "band_width": b, "parallelism": "replicas only",
-                   "l2": "inputs larger than L2 (matrix %.1f GB)" % (mat_bytes / 1e9),
-                   "input_regeneration": "device copy outside the timed brackets"},
+        "config": cfg,
         "clocks": clocks, "e2e": e2e, "gpu_launches": launches, "phases": phase_report, "roofline": roofline,
         "cpu_baseline": cpu, "validity": valid, "epilogue": epilogue, "context": context,
         "total_tflops": (cw["p1_flops"] + cw["p2_flops"] + cw["p4a_flops"] + cw["p4b_flops"]) / ms_per_step / 1e9,

@@ -40,17 +40,22 @@ typedef struct eigh_handle_s* eigh_handle_t;
  * Defaults: band width b = 64, D&C leaf 32, WY group g = 8. */
 int eigh_create(eigh_handle_t* h, int64_t N, int64_t nev);
 
-/* Tuning knobs; must be called before eigh_workspace_size.  Keys: "band_width" (64 or 128),
- * "wy_group" (reflectors per compact-WY block of S4a: 8, 16 or 32), "dc_leaf" (8..32), "p4b_merge" (1..8 panels of S1 merged into one compact-WY block of S4b; default 4; 8 measures 0.4 % faster at N = 27648),
+/* Tuning knobs.  Keys: "wy_group" (reflectors per compact-WY block of S4a: 8, 16 or 32), "dc_leaf" (8..32),
+ * "p4b_merge" (1..8 panels of S1 merged into one compact-WY block of S4b; default 4),
  * "gemm_3m" (1 = complex GEMMs of S1 / S4b by the 3M method, three real tensor-core products per complex
  * multiply-add, the default; 0 = four products.  The switch is process-wide: handles used concurrently must agree),
  * "panel_smem" (S1.1: 1 = shared-memory resident panel QR with the T factor built in, 0 = L2-resident panel QR + Gram
  * GEMM + T recurrence), "panel_rows_min" (16..192 panel rows per thread block of the resident kernel),
- * "hemm_waves" (S1.3: split-K of HEMM-lower sized for about this many thread blocks per SM; default 14, 7..28 measure within 1 %),
+ * "hemm_waves" (S1.3: split-K of HEMM-lower sized for about this many thread blocks per SM; default 14),
  * "bt_chain" (S4a: consecutive passes of one column slab scheduled back to back so that followers read from L2;
- * 0 = automatic = 1, the unchained order, which measures fastest), "bc_grid" (thread blocks of the S2 bulge-chasing kernel; 0 = every co-resident block, the default).
- * Returns -2 for an unknown key, -3 for a bad value. */
+ * 0 = automatic = 1, the unchained order), "bc_grid" (thread blocks of the S2 bulge-chasing kernel; 0 = every
+ * co-resident block, the default), "band_width" (64: the only width S2 / S4a are built for; anything else is -3).
+ * Changing an option invalidates the workspace: call eigh_workspace_size / eigh_set_workspace again afterwards
+ * (every compute entry point returns -1 until then).  Returns -2 for an unknown key, -3 for a bad value. */
 int eigh_set_option(eigh_handle_t h, const char* key, int64_t value);
+
+/* Current value of an option (same keys as eigh_set_option).  Returns -2 for an unknown key, -3 for value == NULL. */
+int eigh_get_option(eigh_handle_t h, const char* key, int64_t* value);
 
 /* Bytes of device workspace the caller must provide for this plan. */
 size_t eigh_workspace_size(eigh_handle_t h);
@@ -70,11 +75,13 @@ int eigh_set_workspace(eigh_handle_t h, void* ws_dev, size_t bytes);
 int eigh_solve(eigh_handle_t h, void* A_dev, int64_t lda, double* W_dev, void* Z_dev,
                void* stream);
 
-/* The same solve with HOST buffers (end-to-end path): copies A_host (N x N c128, lda >= N,
- * pinned or pageable) to A_scratch_dev, runs eigh_solve, copies W (N doubles) and Z (N x nev
- * c128) back to W_host / Z_host.  A_scratch_dev (lda*N c128), W_scratch_dev (N doubles) and
- * Z_scratch_dev (N*nev c128) are caller-owned device buffers.  A_host is not modified.
- * Synchronises `stream` before returning. */
+/* The same solve with HOST buffers (end-to-end path).  A_host (N x N c128, lda >= N, pageable or pinned; not
+ * modified) is streamed to A_scratch_dev through a bounded, double-buffered pinned staging ring owned by the handle
+ * (2 x 256 MiB, allocated on first use, one cudaMemcpyAsync per chunk, the host-side fill of one buffer overlapping
+ * the transfer of the other); eigh_solve runs; W (N doubles) and Z (N x nev c128) are streamed back to W_host /
+ * Z_host the same way.  No pinned memory proportional to N^2 is needed.  A_scratch_dev (lda*N c128), W_scratch_dev
+ * (N doubles) and Z_scratch_dev (N*nev c128) are caller-owned device buffers.  Uses `stream` and one internal
+ * copy stream; synchronises both before returning. */
 int eigh_solve_host(eigh_handle_t h, const void* A_host, int64_t lda, double* W_host, void* Z_host,
                     void* A_scratch_dev, double* W_scratch_dev, void* Z_scratch_dev, void* stream);
 
@@ -116,11 +123,21 @@ int eigh_band_to_tridiag(eigh_handle_t h, void* band_dev, int64_t ldab, double* 
                          double* e_dev, void* stream);
 
 /* S3 ("diagonalizing this tridiagonal form"), divide and conquer on the GPU.
- * d_dev[N], e_dev[N-1] are read (not modified).  W_dev[N] ascending.  Q_dev: N x nev real
- * FP64, ldq >= N, column j = eigenvector of W[j]; may alias no other argument.
+ * d_dev[N], e_dev[N-1] are read (not modified); e may have either sign (the solver works on |e| and scales row i
+ * of Q by prod_{t<i} sign(e_t), which maps the eigenvectors back to the signed matrix).  W_dev[N] ascending.
+ * Q_dev: N x nev real FP64, ldq >= N, column j = eigenvector of W[j]; may alias no other argument.
  * Synchronises `stream`.  Returns the number of secular roots that failed to converge. */
 int eigh_tridiag_dc(eigh_handle_t h, const double* d_dev, const double* e_dev, double* W_dev,
                     double* Q_dev, int64_t ldq, void* stream);
+
+/* Statistics of the last S3 run on this handle (eigh_tridiag_dc or eigh_solve), per merge level (level 0 = the
+ * merges of pairs of leaves, the last level = the root merge):
+ *   flops_executed[l] = sum over the merge GEMMs of the level of 2 M N K as launched (block structure of Q_old and
+ *                       deflation taken into account: the real FP64 tensor-core flops of S3.5),
+ *   kept_frac[l]      = sum k / sum n over the merges of the level (k = non-deflated values; 1 - kept_frac is the
+ *                       deflation ratio of SURVEY.md 8(d)).
+ * Both arrays hold up to `cap` entries; *nlevels gets the number of levels.  Host pointers. */
+int eigh_dc_stats(eigh_handle_t h, int cap, int* nlevels, double* flops_executed, double* kept_frac);
 
 /* S4a (first of the "two stages"): Z <- Q2 * (phase o Q_T).
  * Q_dev: N x nev real (from S3); Z_dev: N x nev c128, ldz >= N. */
@@ -183,7 +200,7 @@ int eigh_assemble_bdg(eigh_handle_t h, int64_t nx, int64_t ny, int64_t nz, const
                       double mu, double sign, void* A_dev, int64_t lda, void* stream);
 
 /* ---------------------------------------------------------------------------------------
- * Kernel-level entry points (unit tests and microbenchmarks of the building blocks).
+ * Kernel-level entry points (unit tests of the building blocks).
  * ------------------------------------------------------------------------------------- */
 
 /* Complex-FP64 GEMM on the FP64 tensor-core path (mma.sync m8n8k4 f64 -> DMMA):
@@ -209,17 +226,6 @@ int eigh_k_zhemm_lower(eigh_handle_t h, int64_t M, int64_t N, const void* A_dev,
 int eigh_k_dgemm(eigh_handle_t h, int64_t M, int64_t N, int64_t K, const double* A_dev,
                  int64_t lda, const int32_t* a_col_idx_dev, const double* B_dev, int64_t ldb,
                  double* C_dev, int64_t ldc, void* stream);
-
-/* Register-resident DMMA / DFMA peak microbenchmarks: run `iters` dependent-chain-free
- * instructions per thread on every SM; returns achieved real TFLOP/s in *tflops (host). */
-int eigh_k_fp64_peak(int use_dmma, int64_t iters, double* tflops, double* ms, void* stream);
-
-/* Configurable variant: kind 0 = DFMA loop, 1 = mma.sync.m8n8k4.f64 loop, 2 = mma.sync.m16n8k16.f64 loop, with
- * `blocks_per_sm` thread blocks of `threads` threads on every SM; kind 10..13 = the inner loop of the 3M GEMM engine
- * (10: DMMAs on register operands, 11: + shared-memory fragment loads and the 3M adds, 12: + a block barrier per k-block,
- * 13: + the cp.async traffic of a k-block; fixed at 3 blocks of 128 threads per SM).  Returns real TFLOP/s (2 per FMA). */
-int eigh_k_fp64_probe(int kind, int blocks_per_sm, int threads, int64_t iters, double* tflops, double* ms,
-                      void* stream);
 
 #ifdef __cplusplus
 }

@@ -21,6 +21,7 @@ _dp = ctypes.POINTER(ctypes.c_double)
 SIGNATURES = {
     "eigh_create": (_int, [ctypes.POINTER(_vp), _i64, _i64]),
     "eigh_set_option": (_int, [_vp, ctypes.c_char_p, _i64]),
+    "eigh_get_option": (_int, [_vp, ctypes.c_char_p, ctypes.POINTER(_i64)]),
     "eigh_workspace_size": (_sz, [_vp]),
     "eigh_set_workspace": (_int, [_vp, _vp, _sz]),
     "eigh_solve": (_int, [_vp, _vp, _i64, _vp, _vp, _vp]),
@@ -28,6 +29,7 @@ SIGNATURES = {
     "eigh_phase_times": (_int, [_vp, _dp]),
     "eigh_kernel_time": (_int, [_vp, ctypes.c_char_p, _dp]),
     "eigh_launch_count": (_i64, [_vp]),
+    "eigh_dc_stats": (_int, [_vp, _int, ctypes.POINTER(_int), _dp, _dp]),
     "eigh_last_error": (ctypes.c_char_p, [_vp]),
     "eigh_destroy": (_int, [_vp]),
     "eigh_reduce_to_band": (_int, [_vp, _vp, _i64, _vp, _i64, _vp]),
@@ -43,8 +45,6 @@ SIGNATURES = {
                             _i64, _vp, _i64, _vp, _i64, _dbl, _vp, _i64, _int, _int, _vp]),
     "eigh_k_zhemm_lower": (_int, [_vp, _i64, _i64, _vp, _i64, _vp, _i64, _vp, _i64, _int, _vp]),
     "eigh_k_dgemm": (_int, [_vp, _i64, _i64, _i64, _vp, _i64, _vp, _vp, _i64, _vp, _i64, _vp]),
-    "eigh_k_fp64_peak": (_int, [_int, _i64, _dp, _dp, _vp]),
-    "eigh_k_fp64_probe": (_int, [_int, _int, _int, _i64, _dp, _dp, _vp]),
 }
 
 
@@ -225,13 +225,28 @@ class Eigh:
         return int(self.lib.eigh_launch_count(self.h))
 
     # ------------------------------------------------------------------ phases
+    def get_option(self, key: str) -> int:
+        v = _i64()
+        rc = self.lib.eigh_get_option(self.h, key.encode(), ctypes.byref(v))
+        self._check(rc, f"eigh_get_option({key})")
+        return int(v.value)
+
+    def dc_stats(self):
+        """Per merge level of the last S3 run: (executed GEMM flops, kept fraction k/n) -- eigh_dc_stats."""
+        n = _int()
+        fl = (ctypes.c_double * 32)()
+        kf = (ctypes.c_double * 32)()
+        rc = self.lib.eigh_dc_stats(self.h, 32, ctypes.byref(n), fl, kf)
+        self._check(rc, "eigh_dc_stats")
+        return [float(fl[i]) for i in range(min(n.value, 32))], [float(kf[i]) for i in range(min(n.value, 32))]
+
     @property
     def ldab(self) -> int:
         return 2 * self.band_width + 2
 
     @property
     def band_width(self) -> int:
-        return getattr(self, "_b", 64)
+        return self.get_option("band_width")
 
     def reduce_to_band(self, At, band):
         rc = self.lib.eigh_reduce_to_band(self.h, _ptr(At), self.N, _ptr(band), band.shape[1], _stream())
@@ -270,24 +285,3 @@ class Eigh:
         rc = self.lib.eigh_k_dgemm(self.h, M, N, K, _ptr(A), lda, _ptr(col_idx), _ptr(B), ldb, _ptr(C), ldc,
                                    _stream())
         self._check(rc, "eigh_k_dgemm")
-
-
-def fp64_peak(use_dmma: bool, iters: int = 20000):
-    """(TFLOP/s, ms) of the register-resident DMMA (or DFMA) loop on the current device."""
-    lib = load()
-    tf, ms = ctypes.c_double(), ctypes.c_double()
-    rc = lib.eigh_k_fp64_peak(1 if use_dmma else 0, iters, ctypes.byref(tf), ctypes.byref(ms), _stream())
-    if rc != 0:
-        raise EighError(f"eigh_k_fp64_peak -> {rc}")
-    return tf.value, ms.value
-
-
-def fp64_probe(kind: int, blocks_per_sm: int = 2, threads: int = 256, iters: int = 20000):
-    """(TFLOP/s, ms) of one configuration of the FP64 microbenchmarks (eigh_k_fp64_probe)."""
-    lib = load()
-    tf, ms = ctypes.c_double(), ctypes.c_double()
-    rc = lib.eigh_k_fp64_probe(int(kind), int(blocks_per_sm), int(threads), int(iters), ctypes.byref(tf), ctypes.byref(ms),
-                               _stream())
-    if rc != 0:
-        raise EighError(f"eigh_k_fp64_probe -> {rc}")
-    return tf.value, ms.value

@@ -4,6 +4,10 @@
 
 #include <algorithm>
 #include <new>
+#include <thread>
+#include <vector>
+
+#include <nvtx3/nvToolsExt.h>
 
 #include "dgemm.cuh"
 #include "eigh_internal.h"
@@ -116,13 +120,13 @@ int eigh_set_option(eigh_handle_t h, const char* key, int64_t value) {
     if (!h) return -1;
     if (!key) return -2;
     if (!strcmp(key, "band_width")) {
-        if (value != 64 && value != 128) return set_err(h, -3, "band_width must be 64 or 128");
+        if (value != 64) return set_err(h, -3, "band_width must be 64 (the width S2 and S4a are built for)");
         h->b = (int)value;
     } else if (!strcmp(key, "wy_group")) {
         if (value != 8 && value != 16 && value != 32) return set_err(h, -3, "wy_group must be 8, 16 or 32");
         h->g = (int)value;
     } else if (!strcmp(key, "dc_leaf")) {
-        if (value < 4 || value > 32) return set_err(h, -3, "dc_leaf must be in [4, 32]");
+        if (value < 8 || value > 32) return set_err(h, -3, "dc_leaf must be in [8, 32]");
         h->leaf = (int)value;
     } else if (!strcmp(key, "p4b_merge")) {
         if (value < 1 || value > 8) return set_err(h, -3, "p4b_merge must be in [1, 8]");
@@ -148,7 +152,29 @@ int eigh_set_option(eigh_handle_t h, const char* key, int64_t value) {
     } else {
         return set_err(h, -2, "unknown option '%s'", key);
     }
+    // the plan (and with it the size and the layout of the workspace) depends on the options: the workspace handed
+    // over earlier is dropped, so that a buffer sized for the old plan can never be used with the new one
     h->planned = false;
+    h->ws = nullptr;
+    h->ws_bytes = 0;
+    return 0;
+}
+
+int eigh_get_option(eigh_handle_t h, const char* key, int64_t* value) {
+    if (!h) return -1;
+    if (!key) return -2;
+    if (!value) return -3;
+    if (!strcmp(key, "band_width")) *value = h->b;
+    else if (!strcmp(key, "wy_group")) *value = h->g;
+    else if (!strcmp(key, "dc_leaf")) *value = h->leaf;
+    else if (!strcmp(key, "p4b_merge")) *value = h->p4b_merge;
+    else if (!strcmp(key, "gemm_3m")) *value = h->gemm_3m;
+    else if (!strcmp(key, "panel_smem")) *value = h->panel_smem;
+    else if (!strcmp(key, "panel_rows_min")) *value = h->panel_rows_min;
+    else if (!strcmp(key, "bt_chain")) *value = h->bt_chain;
+    else if (!strcmp(key, "hemm_waves")) *value = h->hemm_waves;
+    else if (!strcmp(key, "bc_grid")) *value = h->bc_grid;
+    else return set_err(h, -2, "unknown option '%s'", key);
     return 0;
 }
 
@@ -171,8 +197,10 @@ int eigh_set_workspace(eigh_handle_t h, void* ws_dev, size_t bytes) {
 static int ensure_ready(eigh_handle_t h) {
     if (!h) return -1;
     g_zgemm_3m = h->gemm_3m != 0;            // process-wide switch of the GEMM engine, set from the handle in use
-    if (!h->ws) return set_err(h, -1, "no workspace set (call eigh_set_workspace)");
+    if (!h->ws) return set_err(h, -1, "no workspace set (call eigh_set_workspace; eigh_set_option drops an earlier one)");
     if (!h->planned) return set_err(h, -1, "options changed after eigh_set_workspace; call eigh_workspace_size / eigh_set_workspace again");
+    if (h->ws_bytes < h->plan.total)
+        return set_err(h, -1, "workspace too small for the current plan: %zu < %zu", h->ws_bytes, h->plan.total);
     if (!h->events_ok) {
         for (int i = 0; i < 6; ++i) {
             cudaError_t e = cudaEventCreate(&h->ev[i]);
@@ -192,6 +220,13 @@ static int ensure_ready(eigh_handle_t h) {
     }
     return 0;
 }
+
+namespace {
+struct NvtxRange {
+    explicit NvtxRange(const char* name) { nvtxRangePushA(name); }
+    ~NvtxRange() { nvtxRangePop(); }
+};
+}  // namespace
 
 static int cuda_fail(eigh_handle_t h, int rc, const char* where) {
     if (rc >= 1000) return set_err(h, rc, "%s: CUDA error %d (%s)", where, rc - 1000, cudaGetErrorString((cudaError_t)(rc - 1000)));
@@ -315,20 +350,27 @@ int eigh_solve(eigh_handle_t h, void* A_dev, int64_t lda, double* W_dev, void* Z
     const int64_t ldq = round_up(h->N, 8);
     h->launches = 0;
     int nfail = 0;
+    // NVTX ranges mark the host-side enqueue of every phase (the device-side spans are the CUDA events below)
+    NvtxRange whole("eigh_solve");
     cudaEventRecord(h->ev[0], s);
-    rc = phase_reduce_to_band(h, (c128*)A_dev, lda, band, h->ldab, s);
+    { NvtxRange r("S1 full->band");
+      rc = phase_reduce_to_band(h, (c128*)A_dev, lda, band, h->ldab, s); }
     if (rc) return cuda_fail(h, rc, "reduce_to_band");
     cudaEventRecord(h->ev[1], s);
-    rc = phase_band_to_tridiag(h, band, h->ldab, d, e, s);
+    { NvtxRange r("S2 band->tridiagonal");
+      rc = phase_band_to_tridiag(h, band, h->ldab, d, e, s); }
     if (rc) return cuda_fail(h, rc, "band_to_tridiag");
     cudaEventRecord(h->ev[2], s);
-    rc = phase_tridiag_dc(h, d, e, W_dev, Qt, ldq, s, &nfail);
+    { NvtxRange r("S3 tridiagonal D&C");
+      rc = phase_tridiag_dc(h, d, e, W_dev, Qt, ldq, s, &nfail); }
     if (rc) return cuda_fail(h, rc, "tridiag_dc");
     cudaEventRecord(h->ev[3], s);
-    rc = phase_backtransform_band(h, Qt, ldq, (c128*)Z_dev, h->N, s);
+    { NvtxRange r("S4a band back-transform");
+      rc = phase_backtransform_band(h, Qt, ldq, (c128*)Z_dev, h->N, s); }
     if (rc) return cuda_fail(h, rc, "backtransform_band");
     cudaEventRecord(h->ev[4], s);
-    rc = phase_backtransform_full(h, (const c128*)A_dev, lda, (c128*)Z_dev, h->N, s);
+    { NvtxRange r("S4b full back-transform");
+      rc = phase_backtransform_full(h, (const c128*)A_dev, lda, (c128*)Z_dev, h->N, s); }
     if (rc) return cuda_fail(h, rc, "backtransform_full");
     cudaEventRecord(h->ev[5], s);
     cudaError_t ce = cudaStreamSynchronize(s);
@@ -348,6 +390,103 @@ int eigh_solve(eigh_handle_t h, void* A_dev, int64_t lda, double* W_dev, void* Z
     return nfail;
 }
 
+// ---- eigh_solve_host: host <-> device streaming through a bounded pinned ring -----------------------------------
+constexpr size_t STAGE_BYTES = (size_t)256 << 20;
+
+static int stage_init(eigh_handle_s* h) {
+    if (h->stage_ok) return 0;
+    for (int i = 0; i < 2; ++i) {
+        cudaError_t e = cudaMallocHost(&h->stage[i], STAGE_BYTES);
+        if (e == cudaSuccess) e = cudaEventCreateWithFlags(&h->ev_stage[i], cudaEventDisableTiming);
+        if (e != cudaSuccess) return set_err(h, 1000 + (int)e, "eigh_solve_host staging ring: %s", cudaGetErrorString(e));
+    }
+    cudaError_t e = cudaStreamCreateWithFlags(&h->copy_stream, cudaStreamNonBlocking);
+    if (e != cudaSuccess) return set_err(h, 1000 + (int)e, "eigh_solve_host copy stream: %s", cudaGetErrorString(e));
+    h->stage_bytes = STAGE_BYTES;
+    h->stage_ok = true;
+    return 0;
+}
+
+static bool host_is_pinned(const void* p) {
+    cudaPointerAttributes at;
+    if (cudaPointerGetAttributes(&at, p) != cudaSuccess) { (void)cudaGetLastError(); return false; }
+    return at.type == cudaMemoryTypeHost;
+}
+
+// plain host copy split over a few threads (a single thread fills the ring slower than PCIe drains it)
+static void host_copy(void* dst, const void* src, size_t bytes) {
+    const int nt = bytes >= ((size_t)8 << 20) ? 8 : 1;
+    if (nt == 1) { memcpy(dst, src, bytes); return; }
+    std::vector<std::thread> th;
+    const size_t per = ((bytes + nt - 1) / nt + 63) / 64 * 64;
+    for (int t = 0; t < nt; ++t) {
+        const size_t off = (size_t)t * per;
+        if (off >= bytes) break;
+        const size_t n = std::min(per, bytes - off);
+        th.emplace_back([=] { memcpy((char*)dst + off, (const char*)src + off, n); });
+    }
+    for (auto& t : th) t.join();
+}
+
+// host -> device, `bytes` contiguous.  Pinned source: chunked direct copies.  Pageable source: the ring, the fill of
+// one buffer overlapping the transfer of the other.  All copies on `cs`.
+static cudaError_t stream_h2d(eigh_handle_s* h, void* dst_dev, const void* src_host, size_t bytes, cudaStream_t cs) {
+    const bool pinned = host_is_pinned(src_host);
+    size_t off = 0;
+    for (int i = 0; off < bytes; ++i) {
+        const size_t n = std::min(h->stage_bytes, bytes - off);
+        cudaError_t e;
+        if (pinned) {
+            e = cudaMemcpyAsync((char*)dst_dev + off, (const char*)src_host + off, n, cudaMemcpyHostToDevice, cs);
+        } else {
+            const int b = i & 1;
+            e = cudaEventSynchronize(h->ev_stage[b]);          // the transfer that last used this buffer is done
+            if (e != cudaSuccess) return e;
+            host_copy(h->stage[b], (const char*)src_host + off, n);
+            e = cudaMemcpyAsync((char*)dst_dev + off, h->stage[b], n, cudaMemcpyHostToDevice, cs);
+            if (e == cudaSuccess) e = cudaEventRecord(h->ev_stage[b], cs);
+        }
+        if (e != cudaSuccess) return e;
+        off += n;
+    }
+    return cudaSuccess;
+}
+
+// device -> host, `bytes` contiguous; the host-side drain of chunk i-1 overlaps the transfer of chunk i.
+static cudaError_t stream_d2h(eigh_handle_s* h, void* dst_host, const void* src_dev, size_t bytes, cudaStream_t cs) {
+    if (host_is_pinned(dst_host)) {
+        for (size_t off = 0; off < bytes; off += h->stage_bytes) {
+            const size_t n = std::min(h->stage_bytes, bytes - off);
+            cudaError_t e = cudaMemcpyAsync((char*)dst_host + off, (const char*)src_dev + off, n, cudaMemcpyDeviceToHost, cs);
+            if (e != cudaSuccess) return e;
+        }
+        return cudaSuccess;
+    }
+    size_t off = 0, prev_off = 0, prev_n = 0;
+    int i = 0;
+    for (; off < bytes; ++i) {
+        const size_t n = std::min(h->stage_bytes, bytes - off);
+        const int b = i & 1;
+        cudaError_t e = cudaMemcpyAsync(h->stage[b], (const char*)src_dev + off, n, cudaMemcpyDeviceToHost, cs);
+        if (e == cudaSuccess) e = cudaEventRecord(h->ev_stage[b], cs);
+        if (e != cudaSuccess) return e;
+        if (prev_n) {
+            e = cudaEventSynchronize(h->ev_stage[b ^ 1]);
+            if (e != cudaSuccess) return e;
+            host_copy((char*)dst_host + prev_off, h->stage[b ^ 1], prev_n);
+        }
+        prev_off = off; prev_n = n;
+        off += n;
+    }
+    if (prev_n) {
+        const int b = (i - 1) & 1;
+        cudaError_t e = cudaEventSynchronize(h->ev_stage[b]);
+        if (e != cudaSuccess) return e;
+        host_copy((char*)dst_host + prev_off, h->stage[b], prev_n);
+    }
+    return cudaSuccess;
+}
+
 int eigh_solve_host(eigh_handle_t h, const void* A_host, int64_t lda, double* W_host, void* Z_host,
                     void* A_scratch_dev, double* W_scratch_dev, void* Z_scratch_dev, void* stream) {
     int rc = ensure_ready(h);
@@ -359,17 +498,43 @@ int eigh_solve_host(eigh_handle_t h, const void* A_host, int64_t lda, double* W_
     if (!A_scratch_dev) return -6;
     if (!W_scratch_dev) return -7;
     if (!Z_scratch_dev) return -8;
+    rc = stage_init(h);
+    if (rc) return rc;
     cudaStream_t s = (cudaStream_t)stream;
-    cudaError_t ce = cudaMemcpyAsync(A_scratch_dev, A_host, (size_t)lda * h->N * sizeof(c128), cudaMemcpyHostToDevice, s);
+    NvtxRange whole("eigh_solve_host");
+    // the copies run on the handle's copy stream, ordered against the caller's stream by events
+    cudaError_t ce = cudaEventRecord(h->ev[0], s);
+    if (ce == cudaSuccess) ce = cudaStreamWaitEvent(h->copy_stream, h->ev[0], 0);
+    if (ce == cudaSuccess) {
+        NvtxRange r("H2D A");
+        ce = stream_h2d(h, A_scratch_dev, A_host, (size_t)lda * h->N * sizeof(c128), h->copy_stream);
+    }
+    if (ce == cudaSuccess) ce = cudaEventRecord(h->ev[1], h->copy_stream);
+    if (ce == cudaSuccess) ce = cudaStreamWaitEvent(s, h->ev[1], 0);
     if (ce != cudaSuccess) return set_err(h, 1000 + (int)ce, "eigh_solve_host H2D: %s", cudaGetErrorString(ce));
-    rc = eigh_solve(h, A_scratch_dev, lda, W_scratch_dev, Z_scratch_dev, stream);
+    rc = eigh_solve(h, A_scratch_dev, lda, W_scratch_dev, Z_scratch_dev, stream);     // synchronises `stream`
     if (rc < 0 || rc >= 1000) return rc;
-    ce = cudaMemcpyAsync(W_host, W_scratch_dev, (size_t)h->N * sizeof(double), cudaMemcpyDeviceToHost, s);
-    if (ce == cudaSuccess)
-        ce = cudaMemcpyAsync(Z_host, Z_scratch_dev, (size_t)h->N * h->nev * sizeof(c128), cudaMemcpyDeviceToHost, s);
-    if (ce == cudaSuccess) ce = cudaStreamSynchronize(s);
+    {
+        NvtxRange r("D2H W, Z");
+        ce = stream_d2h(h, W_host, W_scratch_dev, (size_t)h->N * sizeof(double), h->copy_stream);
+        if (ce == cudaSuccess)
+            ce = stream_d2h(h, Z_host, Z_scratch_dev, (size_t)h->N * h->nev * sizeof(c128), h->copy_stream);
+    }
+    if (ce == cudaSuccess) ce = cudaStreamSynchronize(h->copy_stream);
     if (ce != cudaSuccess) return set_err(h, 1000 + (int)ce, "eigh_solve_host D2H: %s", cudaGetErrorString(ce));
     return rc;
+}
+
+int eigh_dc_stats(eigh_handle_t h, int cap, int* nlevels, double* flops_executed, double* kept_frac) {
+    if (!h) return -1;
+    if (cap < 0) return -2;
+    if (!nlevels) return -3;
+    *nlevels = h->dc_levels;
+    for (int l = 0; l < h->dc_levels && l < cap; ++l) {
+        if (flops_executed) flops_executed[l] = h->dc_flops[l];
+        if (kept_frac) kept_frac[l] = h->dc_nsum[l] > 0.0 ? h->dc_ksum[l] / h->dc_nsum[l] : 0.0;
+    }
+    return 0;
 }
 
 int eigh_phase_times(eigh_handle_t h, double ms[5]) {
@@ -397,6 +562,12 @@ int eigh_destroy(eigh_handle_t h) {
     {
         for (int i = 0; i < 6; ++i) cudaEventDestroy(h->ev[i]);
         for (int i = 0; i < 2; ++i) cudaEventDestroy(h->ev_sweep[i]);
+    }
+    if (h->stage_ok) {
+        for (int i = 0; i < 2; ++i) { cudaFreeHost(h->stage[i]); cudaEventDestroy(h->ev_stage[i]); }
+        cudaStreamDestroy(h->copy_stream);
+    } else {
+        for (int i = 0; i < 2; ++i) if (h->stage[i]) cudaFreeHost(h->stage[i]);
     }
     delete h;
     return 0;

@@ -488,12 +488,9 @@ int phase_reduce_to_band(eigh_handle_s* h, c128* A, int64_t lda, c128* band, int
     const size_t ps_smem = (size_t)(PS_MAXROWS * PS_LD + 4 * PS_B + 3 * PS_B) * sizeof(c128);
     const size_t pq_smem = (size_t)(PQ_WARPS * b + b + 4) * sizeof(c128);
     const size_t tf_smem = (size_t)(2 * b * (b + 1) + b) * sizeof(c128);
-    static bool attr = false;
-    if (!attr) {
-        EIGH_CUDA_OK(cudaFuncSetAttribute(tfactor_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)tf_smem));
-        EIGH_CUDA_OK(cudaFuncSetAttribute(panel_qr_smem_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ps_smem));
-        attr = true;
-    }
+    // (set on every call: the attribute is per device / context, and the call is cheap)
+    EIGH_CUDA_OK(cudaFuncSetAttribute(tfactor_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)tf_smem));
+    EIGH_CUDA_OK(cudaFuncSetAttribute(panel_qr_smem_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ps_smem));
     int max_coop = 0;
     EIGH_CUDA_OK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&max_coop, panel_qr_kernel, PQ_NT, pq_smem));
     if (max_coop < 1) return set_err(h, EIGH_ERR_CUDA, "panel_qr_kernel cannot be resident");
@@ -565,7 +562,8 @@ int phase_reduce_to_band(eigh_handle_s* h, c128* A, int64_t lda, c128* band, int
     }
     extract_band_kernel<<<N, 128, 0, s>>>(A, lda, N, b, band, ldab);
     ++h->launches;
-    return (int)cudaGetLastError() ? 1000 + (int)cudaGetLastError() : 0;
+    const cudaError_t ce = cudaGetLastError();
+    return ce != cudaSuccess ? 1000 + (int)ce : 0;
 }
 
 }  // namespace eigh

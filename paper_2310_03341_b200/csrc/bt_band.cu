@@ -43,12 +43,8 @@
 
 namespace eigh {
 
-#ifndef BT_QPLANE
-#define BT_QPLANE 1      // stage tiles carry q = vx - vy (a third bulk copy, 16 KB): no V-side adds in the two 3-product forms
-#endif
-#ifndef BT_RING8
-#define BT_RING8 (BT_QPLANE ? 3 : 4)
-#endif
+constexpr bool BT_QPLANE = true;    // stage tiles carry q = vx - vy (a third bulk copy, 16 KB): no V-side adds in the two 3-product forms
+constexpr int BT_RING8 = 3;         // stages of the ring for GS = 8 (with the q plane there is room for three)
 constexpr int BT_B = 64;            // band width (reflector length)
 constexpr int BT_P = 32;            // sweeps per pass
 constexpr int BT_WR = BT_B + BT_P;  // window rows (96)
@@ -225,13 +221,6 @@ __device__ __forceinline__ void dmma_p(double (&c)[2], double a, double b) {
         : "d"(a), "d"(b));
 }
 
-#ifndef BT_GAUSS2
-#define BT_GAUSS2 1
-#endif
-#ifndef BT_3M1
-#define BT_3M1 1
-#endif
-
 // q = Re v - Im v for every stored reflector element (the third operand of the 3-product forms, formed once here instead
 // of once per warp and use inside the sweep)
 __global__ void bt_vq_kernel(const c128* __restrict__ V2, double* __restrict__ q, int64_t n) {
@@ -304,17 +293,9 @@ __device__ __forceinline__ void bt_apply_step(const c128* __restrict__ Vs, const
                             if constexpr (bt_qplane(GS)) qv = Qs[(8 * p + 2 * t + h) + (8 * cb + g) * BT_LDV];
                         }
                         if constexpr (!bt_qplane(GS)) qv = v.x - v.y;
-#if BT_3M1
                         dmma_p(s1[c][h], ar, v.x);
                         dmma_p(s2[c][h], ai, v.y);
                         dmma_p(s3[c][h], as, qv);
-#else
-                        // four products: s1 = Re = sum ar vx + ai vy,  s3 = Im = sum ai vx - ar vy  (s2 stays zero)
-                        dmma_p(s1[c][h], ar, v.x);
-                        dmma_p(s1[c][h], ai, v.y);
-                        dmma_p(s3[c][h], ai, v.x);
-                        dmma_p(s3[c][h], ar, -v.y);
-#endif
                     }
                 }
             }
@@ -325,13 +306,8 @@ __device__ __forceinline__ void bt_apply_step(const c128* __restrict__ Vs, const
 #pragma unroll
             for (int e = 0; e < 2; ++e) {
                 const double t1 = s1[c][0][e] + s1[c][1][e], t2 = s2[c][0][e] + s2[c][1][e], t3 = s3[c][0][e] + s3[c][1][e];
-#if BT_3M1
                 ar1[c][e] = t1 + t2;
                 ai1[c][e] = (t3 - t1) + t2;
-#else
-                ar1[c][e] = t1 + t2;          // t2 = 0
-                ai1[c][e] = t3;
-#endif
             }
         // ---- Y = (-T) Y1   (m = column of Z, n = output reflector, k = input reflector >= output)
         double yr[NB][2], yi[NB][2];
@@ -384,7 +360,6 @@ __device__ __forceinline__ void bt_apply_step(const c128* __restrict__ Vs, const
             }
         }
         } else {
-#if BT_GAUSS2
         // Three real products per complex multiply-add (Gauss): with y = ar + i ai and v = vx + i vy,
         //   k1 = ar (vx + vy),  k2 = (ai - ar) vx,  k3 = (ar + ai) vy;   Re(y v) = k1 - k3,  Im(y v) = k1 + k2.
         // k2 and k3 accumulate straight into zi and zr; k1 is summed over the block's 8 reflectors and added to both.
@@ -414,26 +389,6 @@ __device__ __forceinline__ void bt_apply_step(const c128* __restrict__ Vs, const
                 zi[p][0] += k1[0]; zi[p][1] += k1[1];
             }
         }
-#else
-#pragma unroll
-        for (int c = 0; c < NB; ++c) {
-            const int cb = cb0 + c;
-#pragma unroll
-            for (int h = 0; h < 2; ++h) {
-                const double ar = yr[c][h], ai = yi[c][h], nai = -ai;
-#pragma unroll
-                for (int p = cb; p <= cb + 8; ++p) {
-                    c128 v = cmake(0.0, 0.0);
-                    if ((p != cb || g >= 2 * t + h) && (p != cb + 8 || g < 2 * t + h))
-                        v = Vs[(8 * p + g) + (8 * cb + 2 * t + h) * BT_LDV];
-                    dmma_p(zr[p], ar, v.x);
-                    dmma_p(zi[p], ai, v.x);
-                    dmma_p(zr[p], nai, v.y);
-                    dmma_p(zi[p], ar, v.y);
-                }
-            }
-        }
-#endif
         }
         if (tail) {
             // rows beyond the matrix are virtual: keep them zero (stale V rows may have touched them)
@@ -671,11 +626,9 @@ __global__ void __launch_bounds__(BT_NT, 1) bt_sweep_kernel(const BtSweepArgs a)
 template <int GS>
 static int bt_launch_sweep(eigh_handle_s* h, const BtSweepArgs& a, cudaStream_t s) {
     auto kern = bt_sweep_kernel<GS>;
-    static bool attr = false;
-    if (!attr) {
+    {
         cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bt_smem(GS));
         if (e != cudaSuccess) return 1000 + (int)e;
-        attr = true;
     }
     int grid = h->num_sms;
     const long long units = (long long)a.npass * a.nslabs;
@@ -717,11 +670,7 @@ int phase_backtransform_band(eigh_handle_s* h, const double* Qt, int64_t ldq, c1
     int gs = h->g;
     if (gs != 8 && gs != 16 && gs != 32) gs = 8;
     const size_t tp_smem = (size_t)(BT_WR * BT_P + 2 * BT_P * (BT_P + 1) + BT_P) * sizeof(c128);
-    static bool tp_attr = false;
-    if (!tp_attr) {
-        EIGH_CUDA_OK(cudaFuncSetAttribute(bt_tprep_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)tp_smem));
-        tp_attr = true;
-    }
+    EIGH_CUDA_OK(cudaFuncSetAttribute(bt_tprep_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)tp_smem));
     bt_tprep_kernel<<<dim3((unsigned)kmax, (unsigned)npass), 128, tp_smem, s>>>(ws_ptr<c128>(h, pl.V2), ws_ptr<c128>(h, pl.tau2),
                                                                            kmax, N, gs, pass_off, Tneg);
     h->launches += 2;

@@ -111,20 +111,10 @@ __device__ __forceinline__ void bc_handoff_wait(int odd) {
     else asm volatile("bar.sync 2, %0;" ::"n"(BC_NT + 32) : "memory");
 }
 
-#ifdef BC_PROFILE
-__device__ unsigned long long g_bc_prof[16];
-#define BC_STAMP(i) do { if (t.tid == 0) { const long long now_ = clock64(); atomicAdd(&g_bc_prof[i], (unsigned long long)(now_ - t.last)); t.last = now_; } } while (0)
-#else
-#define BC_STAMP(i) do { } while (0)
-#endif
-
 struct BcStepCtx {
     c128* band; int64_t ldab;
     c128* Vj; c128* tau2j;
     int r, q, rl, lane, warp, tid;
-#ifdef BC_PROFILE
-    mutable long long last;
-#endif
 };
 
 // LAPACK zlarfg on a vector spread over the rows (x = element r, zero for r >= len; all four q lanes of
@@ -174,10 +164,8 @@ __device__ __forceinline__ bool bc_step(BcSmem& sm, const BcStepCtx& t, int r0, 
             if (FULL || (r < len2 && q + 4 * i < len)) sreg[i] = __ldcg(sp + (int64_t)i * 4 * (ldab - 1));
         }
     }
-    BC_STAMP(1);
     cp_async_wait<0>();
     bc_sync_compute();                                   // D landed; vs of this step visible
-    BC_STAMP(2);
     c128 vc[BC_NC];
 #pragma unroll
     for (int i = 0; i < BC_NC; ++i) vc[i] = sm.vs[q + 4 * i];
@@ -229,9 +217,7 @@ __device__ __forceinline__ bool bc_step(BcSmem& sm, const BcStepCtx& t, int r0, 
         if (q == 0) sm.ws[r] = wr;
         if (r == 0 && q == 0) sm.xs[0] = xs0;
     }
-    BC_STAMP(3);
     bc_sync_compute();
-    BC_STAMP(4);
     // ---- next reflector (zlarfg scalars, redundantly in every thread)
     c128 taun = cmake(0.0, 0.0);
     double betan = 0.0;
@@ -278,7 +264,6 @@ __device__ __forceinline__ bool bc_step(BcSmem& sm, const BcStepCtx& t, int r0, 
     bc_handoff_arrive(hb);
     hb ^= 1;
     if (!has_s) return false;
-    BC_STAMP(5);
     // ---- z_c = vn^H S[:, c]: per-thread products, reduce-scatter over the 8 row lanes, then across warps
     {
         c128 zp[BC_NC];
@@ -300,7 +285,6 @@ __device__ __forceinline__ bool bc_step(BcSmem& sm, const BcStepCtx& t, int r0, 
         sm.zpart[t.warp * BC_B + q + 4 * (ibase + 0)] = zp[0];
         sm.zpart[t.warp * BC_B + q + 4 * (ibase + 1)] = zp[1];
     }
-    BC_STAMP(6);
     bc_sync_compute();
     if (t.tid < BC_B) {
         c128 z0 = cadd(sm.zpart[0 * BC_B + t.tid], sm.zpart[1 * BC_B + t.tid]);
@@ -310,7 +294,6 @@ __device__ __forceinline__ bool bc_step(BcSmem& sm, const BcStepCtx& t, int r0, 
         sm.zs[t.tid] = cmulc(taun, cadd(cadd(z0, z1), cadd(z2, z3)));        // conj(tau') z_c
     }
     bc_sync_compute();
-    BC_STAMP(7);
     // ---- S[:, c] -= vn (conj(tau') z_c) for c >= 1; S[:, 0] = beta' e_1; store S and the reflector
     {
         c128* sp = band + (BC_B + r - q) + (int64_t)(r0 + q) * ldab;
@@ -334,7 +317,6 @@ __device__ __forceinline__ bool bc_step(BcSmem& sm, const BcStepCtx& t, int r0, 
     }
     if (t.tid == 0) t.tau2j[k + 1] = taun;
     tau = taun;
-    BC_STAMP(8);
     return true;
 }
 
@@ -401,7 +383,6 @@ __global__ void __launch_bounds__(BC_NT + 32, 1) bulge_chase_kernel(const BcArgs
             if (!more) break;
             if (tid == 0) bc_poll(a.progress, j - 1, k + 3);
             bc_sync_compute();
-            BC_STAMP(9);
         }
     }
 }
@@ -437,11 +418,7 @@ int phase_band_to_tridiag(eigh_handle_s* h, c128* band, int64_t ldab, double* d,
     }
     if (N >= 2) {
         const size_t smem = sizeof(BcSmem);
-        static bool attr = false;
-        if (!attr) {
-            EIGH_CUDA_OK(cudaFuncSetAttribute(bulge_chase_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-            attr = true;
-        }
+        EIGH_CUDA_OK(cudaFuncSetAttribute(bulge_chase_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
         int occ = 0;
         EIGH_CUDA_OK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, bulge_chase_kernel, BC_NT + 32, smem));
         if (occ < 1) return set_err(h, EIGH_ERR_CUDA, "bulge_chase_kernel cannot be resident");
@@ -463,16 +440,3 @@ int phase_band_to_tridiag(eigh_handle_s* h, c128* band, int64_t ldab, double* d,
 }
 
 }  // namespace eigh
-
-#ifdef BC_PROFILE
-// developer-only build (-DBC_PROFILE): cycles accumulated between the stamps of bc_step, CTA-thread 0 of every block
-extern "C" int eigh_debug_bc_profile(unsigned long long out[16], int reset) {
-    cudaDeviceSynchronize();
-    cudaMemcpyFromSymbol(out, eigh::g_bc_prof, 16 * sizeof(unsigned long long));
-    if (reset) {
-        unsigned long long z[16] = {0};
-        cudaMemcpyToSymbol(eigh::g_bc_prof, z, sizeof(z));
-    }
-    return 0;
-}
-#endif

@@ -61,6 +61,15 @@ struct eigh_handle_s {
     double sweep_ms;
     bool events_ok;
     int num_sms;
+    // statistics of the last S3 run, per merge level (eigh_dc_stats)
+    int dc_levels;
+    double dc_flops[32], dc_ksum[32], dc_nsum[32];
+    // eigh_solve_host: bounded pinned staging ring (2 buffers) + its events and copy stream, allocated on first use
+    void* stage[2];
+    size_t stage_bytes;
+    cudaEvent_t ev_stage[2];
+    cudaStream_t copy_stream;
+    bool stage_ok;
 };
 
 namespace eigh {

@@ -33,7 +33,7 @@ constexpr int DC_LEAF_MAX = 32;
 // ------------------------------------------------------------------ arena
 struct DcBufs {
     double *QA, *QB, *U;              // ldq x N each
-    double *dcur, *dnew, *z, *dk, *zk, *mu, *lam, *zhat, *rot_c, *rot_s, *rho, *zsum;
+    double *dcur, *dnew, *z, *dk, *zk, *mu, *lam, *zhat, *rot_c, *rot_s, *rho, *zsum, *esgn, *stats;
     int *perm, *nd_idx, *df_idx, *org, *rot_a, *rot_b, *kcount, *nrot, *fail, *bnd;
     int *ctype, *ktype, *upos, *acol, *k1c, *k2c;   // block structure of Q_old (column types, U row order)
     MergeDesc* desc;                  // all levels, concatenated
@@ -69,6 +69,8 @@ static DcBufs dc_carve(void* base, int64_t N) {
     b.dk = (double*)take(nd); b.zk = (double*)take(nd); b.mu = (double*)take(nd);
     b.lam = (double*)take(nd); b.zhat = (double*)take(nd); b.rot_c = (double*)take(nd);
     b.rot_s = (double*)take(nd); b.rho = (double*)take(nd); b.zsum = (double*)take(nd);
+    b.esgn = (double*)take(nd);
+    b.stats = (double*)take(32 * 3 * sizeof(double));
     b.perm = (int*)take(ni); b.nd_idx = (int*)take(ni); b.df_idx = (int*)take(ni); b.org = (int*)take(ni);
     b.rot_a = (int*)take(ni); b.rot_b = (int*)take(ni); b.kcount = (int*)take(ni); b.nrot = (int*)take(ni);
     b.fail = (int*)take(256); b.bnd = (int*)take(ni);
@@ -93,6 +95,31 @@ __global__ void dc_tear2_kernel(const double* __restrict__ e_in, const int* __re
         const double r = fabs(e_in[m - 1]);
         dcur[m - 1] -= r;
         dcur[m] -= r;
+    }
+}
+
+// The solver works on |e|: T(d, e) = D T(d, |e|) D with D = diag(sgn), sgn_0 = 1, sgn_{i+1} = sgn_i sign(e_i), so the
+// eigenvectors of the signed matrix are the rows of Q scaled by sgn (applied in dc_output_kernel).  One thread block:
+// every thread counts the negative entries of its contiguous chunk, a block scan gives the parity at its start.
+__global__ void __launch_bounds__(1024) dc_esign_kernel(const double* __restrict__ e_in, int N, double* __restrict__ esgn) {
+    __shared__ int cnt[1024];
+    const int tid = threadIdx.x;
+    const int per = (N + 1023) / 1024;
+    const int lo = tid * per, hi = min(N, lo + per);       // sgn[i] for i in [lo, hi) needs e[0 .. i-1]
+    int c = 0;
+    for (int i = lo; i < hi; ++i) c += (i >= 1 && e_in[i - 1] < 0.0) ? 1 : 0;
+    cnt[tid] = c;
+    __syncthreads();
+    for (int o = 1; o < 1024; o <<= 1) {                     // inclusive scan
+        const int v = (tid >= o) ? cnt[tid - o] : 0;
+        __syncthreads();
+        cnt[tid] += v;
+        __syncthreads();
+    }
+    int par = (cnt[tid] - c) & 1;                            // negatives before this chunk
+    for (int i = lo; i < hi; ++i) {
+        if (i >= 1 && e_in[i - 1] < 0.0) par ^= 1;
+        esgn[i] = par ? -1.0 : 1.0;
     }
 }
 
@@ -532,9 +559,10 @@ __global__ void __launch_bounds__(256) dc_wanted_kernel(const MergeDesc* __restr
     if (below < nev) atomicMax(kn, j + 1);
 }
 
+// (also accumulates the level's statistics for eigh_dc_stats: executed GEMM flops, sum of k, sum of n)
 __global__ void dc_gemm_desc_kernel(const MergeDesc* __restrict__ desc, const int* __restrict__ kcount,
                                     const int* __restrict__ k1c, const int* __restrict__ k2c, int nmerge, int64_t ldq,
-                                    DgemmDesc* __restrict__ g, const int* __restrict__ kn) {
+                                    DgemmDesc* __restrict__ g, const int* __restrict__ kn, double* __restrict__ stats) {
     const int mi = blockIdx.x * blockDim.x + threadIdx.x;
     if (mi >= nmerge) return;
     const MergeDesc m = desc[mi];
@@ -557,6 +585,10 @@ __global__ void dc_gemm_desc_kernel(const MergeDesc* __restrict__ desc, const in
     d.M = m.e - m.mid;
     d.K = k - k1e;
     g[2 * mi + 1] = d;
+    const double ncols = (double)d.N;
+    atomicAdd(stats + 0, 2.0 * ncols * ((double)(m.mid - m.s) * (k1 + k2) + (double)(m.e - m.mid) * (k - k1e)));
+    atomicAdd(stats + 1, (double)k);
+    atomicAdd(stats + 2, (double)(m.e - m.s));
 }
 
 __global__ void __launch_bounds__(256) dc_finish_kernel(const MergeDesc* __restrict__ desc, const int* __restrict__ kcount,
@@ -583,14 +615,15 @@ __global__ void __launch_bounds__(256) dc_finish_kernel(const MergeDesc* __restr
 // final: W[rank] = d, Qout[:, rank] = Q[:, j] for rank < nev
 __global__ void __launch_bounds__(256) dc_output_kernel(int N, int nev, const int* __restrict__ perm, const double* __restrict__ dcur,
                                                         const double* __restrict__ Q, int64_t ldq, double* __restrict__ W,
-                                                        double* __restrict__ Qout, int64_t ldo) {
+                                                        double* __restrict__ Qout, int64_t ldo,
+                                                        const double* __restrict__ esgn) {
     const int rank = blockIdx.x;
     const int j = perm[rank];
     if (threadIdx.x == 0) W[rank] = dcur[j];
     if (rank >= nev) return;
     const double* a = Q + (int64_t)j * ldq;
     double* b = Qout + (int64_t)rank * ldo;
-    for (int r = threadIdx.x; r < N; r += 256) b[r] = a[r];
+    for (int r = threadIdx.x; r < N; r += 256) b[r] = esgn[r] * a[r];
 }
 
 // ------------------------------------------------------------------ driver
@@ -634,13 +667,15 @@ int phase_tridiag_dc(eigh_handle_s* h, const double* d, const double* e, double*
     EIGH_CUDA_OK(cudaMemcpyAsync(B.bnd, bnd.data(), (size_t)(L + 1) * sizeof(int), cudaMemcpyHostToDevice, st));
     EIGH_CUDA_OK(cudaMemcpyAsync(B.desc, descs.data(), descs.size() * sizeof(MergeDesc), cudaMemcpyHostToDevice, st));
     EIGH_CUDA_OK(cudaMemsetAsync(B.fail, 0, sizeof(int), st));
+    EIGH_CUDA_OK(cudaMemsetAsync(B.stats, 0, 32 * 3 * sizeof(double), st));
     EIGH_CUDA_OK(cudaStreamSynchronize(st));   // host vectors go out of scope; copies are tiny
 
     // ---- tearing + leaves
     dc_tear_kernel<<<(unsigned)ceil_div(N, 256), 256, 0, st>>>(d, e, N, B.bnd, L, B.dcur);
     dc_tear2_kernel<<<(unsigned)ceil_div(L, 256), 256, 0, st>>>(e, B.bnd, L, B.dcur);
     dc_leaf_kernel<<<(unsigned)ceil_div(L, 4), 128, 0, st>>>(B.bnd, L, B.dcur, e, B.QA, ldq, B.fail);
-    h->launches += 3;
+    dc_esign_kernel<<<1, 1024, 0, st>>>(e, N, B.esgn);
+    h->launches += 4;
 
     double* Qcur = B.QA;
     double* Qnew = B.QB;
@@ -672,7 +707,8 @@ int phase_tridiag_dc(eigh_handle_s* h, const double* d, const double* e, double*
             ++h->launches;
             kn = B.fail + 16;          // second counter in the 256-byte block of `fail`
         }
-        dc_gemm_desc_kernel<<<(unsigned)ceil_div(cnt, 128), 128, 0, st>>>(dd, B.kcount, B.k1c, B.k2c, cnt, ldq, B.gdesc, kn);
+        dc_gemm_desc_kernel<<<(unsigned)ceil_div(cnt, 128), 128, 0, st>>>(dd, B.kcount, B.k1c, B.k2c, cnt, ldq, B.gdesc, kn,
+                                                                          B.stats + 3 * std::min<size_t>(lv, 31));
         h->launches += 9;
         DgemmArgs ga;
         memset(&ga, 0, sizeof(ga));
@@ -687,11 +723,17 @@ int phase_tridiag_dc(eigh_handle_s* h, const double* d, const double* e, double*
     }
     // ---- final ascending order
     dc_rank_kernel<<<dim3((unsigned)ceil_div(N, 256), 1), 256, 0, st>>>(B.desc + final_desc, dcur, B.perm);
-    dc_output_kernel<<<N, 256, 0, st>>>(N, nev, B.perm, dcur, Qcur, ldq, W, Qout, ldo);
+    dc_output_kernel<<<N, 256, 0, st>>>(N, nev, B.perm, dcur, Qcur, ldq, W, Qout, ldo, B.esgn);
     h->launches += 2;
     int fail = 0;
+    double stats[32 * 3];
     EIGH_CUDA_OK(cudaMemcpyAsync(&fail, B.fail, sizeof(int), cudaMemcpyDeviceToHost, st));
+    EIGH_CUDA_OK(cudaMemcpyAsync(stats, B.stats, sizeof(stats), cudaMemcpyDeviceToHost, st));
     EIGH_CUDA_OK(cudaStreamSynchronize(st));
+    h->dc_levels = (int)std::min<size_t>(level_cnt.size(), 32);
+    for (int l = 0; l < h->dc_levels; ++l) {
+        h->dc_flops[l] = stats[3 * l]; h->dc_ksum[l] = stats[3 * l + 1]; h->dc_nsum[l] = stats[3 * l + 2];
+    }
     EIGH_CUDA_OK(cudaGetLastError());
     if (nfail) *nfail = fail;
     return 0;

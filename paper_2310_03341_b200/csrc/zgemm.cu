@@ -7,12 +7,10 @@ template <int WM, int WN, bool TA, bool TB, int MODE, int MINB, int NJ = 4, bool
 static int launch_inst(const ZgemmArgs& a, cudaStream_t stream, int64_t* launches) {
     using Cfg = ZgemmCfg<WM, WN, TA, TB, MODE, NJ>;
     auto kern = zgemm_kernel<WM, WN, TA, TB, MODE, MINB, NJ, M3>;
-    static bool attr_set = false;
-    if (!attr_set) {
+    {   // per device / context, cheap: set on every launch
         cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                              (int)Cfg::SMEM_BYTES);
         if (e != cudaSuccess) return (int)e;
-        attr_set = true;
     }
     dim3 grid((unsigned)((a.M + Cfg::BM - 1) / Cfg::BM), (unsigned)((a.N + Cfg::BN - 1) / Cfg::BN),
               (unsigned)a.splitk);

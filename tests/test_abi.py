@@ -66,3 +66,36 @@ def test_workspace_fits_b200_at_largest_config(lib):
     lib.eigh_destroy(h)
     mat = 49152 * 49152 * 16
     assert ws + 2 * mat < 176e9, (ws + 2 * mat) / 1e9
+
+
+def test_option_change_invalidates_the_workspace(lib):
+    """An option that grows the plan must not be usable with a workspace sized for the old plan
+    (create -> workspace_size -> set_workspace -> set_option -> workspace_size -> solve)."""
+    h = ctypes.c_void_p()
+    assert lib.eigh_create(ctypes.byref(h), 2048, 2048) == 0
+    ws_small = lib.eigh_workspace_size(h)
+    assert lib.eigh_set_workspace(h, ctypes.c_void_p(1 << 20), ws_small) == 0
+    assert lib.eigh_set_option(h, b"p4b_merge", 8) == 0
+    ws_big = lib.eigh_workspace_size(h)
+    assert ws_big > ws_small
+    # nothing may be launched with the old buffer (the pointer is a dummy: a launch would fault)
+    assert lib.eigh_solve(h, ctypes.c_void_p(1 << 20), 2048, ctypes.c_void_p(1 << 20), ctypes.c_void_p(1 << 20), None) == -1
+    assert b"workspace" in lib.eigh_last_error(h)
+    assert lib.eigh_set_workspace(h, ctypes.c_void_p(1 << 20), ws_small) == -3
+    assert lib.eigh_destroy(h) == 0
+
+
+def test_option_ranges_and_get_option(lib):
+    h = ctypes.c_void_p()
+    assert lib.eigh_create(ctypes.byref(h), 512, 512) == 0
+    v = ctypes.c_int64()
+    assert lib.eigh_get_option(h, b"band_width", ctypes.byref(v)) == 0 and v.value == 64
+    assert lib.eigh_set_option(h, b"band_width", 128) == -3      # S2 / S4a are built for 64 only
+    assert lib.eigh_set_option(h, b"dc_leaf", 4) == -3           # documented range 8..32
+    assert lib.eigh_set_option(h, b"dc_leaf", 8) == 0
+    assert lib.eigh_get_option(h, b"dc_leaf", ctypes.byref(v)) == 0 and v.value == 8
+    assert lib.eigh_get_option(h, b"nonsense", ctypes.byref(v)) == -2
+    assert lib.eigh_get_option(h, b"dc_leaf", None) == -3
+    n = ctypes.c_int(-1)
+    assert lib.eigh_dc_stats(h, 0, ctypes.byref(n), None, None) == 0 and n.value == 0
+    assert lib.eigh_destroy(h) == 0

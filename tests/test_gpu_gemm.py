@@ -113,75 +113,3 @@ def test_dgemm(eng, M, N, K):
     eng.dgemm(M, N, K, As, lda, Bs, ldb, Cs2, M)
     torch.cuda.synchronize()
     assert rel(lg(Cs2), A[:M, :K] @ B[:K, :]) < 1e-13
-
-
-def test_fp64_peak_and_gemm_rate(eng):
-    """Not a parity test: records the register-resident DMMA / DFMA rates and the GEMM engine's
-    rates next to cuBLAS in gpurun_out/fp64_peak.json (roofline denominators)."""
-    from paper_2310_03341_b200 import binding
-    out = {}
-    tf, ms = binding.fp64_peak(True, 40000)
-    out["dmma_tflops_burst"] = tf
-    out["dmma_ms"] = ms
-    tf, ms = binding.fp64_peak(False, 40000)
-    out["dfma_tflops_burst"] = tf
-    tf, ms = binding.fp64_peak(True, 2000000)
-    out["dmma_tflops_sustained"] = tf
-    out["dmma_sustained_ms"] = ms
-
-    # DMMA rate against the number of resident warps per SM sub-partition, and the cost of the ingredients of the GEMM
-    # engine's inner loop (eigh_k_fp64_probe; profiles/r01_fp64_peaks.md)
-    for wps, (bps, thr) in {1: (1, 128), 2: (1, 256), 3: (1, 384), 4: (2, 256), 8: (4, 256)}.items():
-        out[f"dmma_tflops_{wps}_warps_per_smsp"] = binding.fp64_probe(1, bps, thr, 20000)[0]
-    out["dmma_m16n8k16_tflops_8_warps_per_smsp"] = binding.fp64_probe(2, 4, 256, 2500)[0]
-    for mode, name in ((10, "dmma_only"), (11, "lds_and_3m_adds"), (12, "barrier"), (13, "cp_async")):
-        out[f"gemm_loop_tflops_{name}"] = binding.fp64_probe(mode, 3, 128, 20000)[0]
-
-    def timeit(fn, n=5):
-        fn()
-        torch.cuda.synchronize()
-        s, e = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-        s.record()
-        for _ in range(n):
-            fn()
-        e.record()
-        torch.cuda.synchronize()
-        return s.elapsed_time(e) / n
-
-    M = N = K = 4096
-    A, B = randc(M, K, 1), randc(K, N, 2)
-    As, Bs = cm(A), cm(B)
-    Cs = torch.zeros((N, M), dtype=torch.complex128, device="cuda")
-    ms = timeit(lambda: eng.zgemm("N", "N", M, N, K, 1.0, As, M, Bs, K, 0.0, Cs, M))
-    out["zgemm_nn_4096_tflops"] = 8.0 * M * N * K / ms / 1e9
-    ms = timeit(lambda: eng.zgemm("N", "C", M, N, K, 1.0, As, M, Bs, K, 0.0, Cs, M))
-    out["zgemm_nc_4096_tflops"] = 8.0 * M * N * K / ms / 1e9
-    ms = timeit(lambda: eng.zgemm("C", "N", M, N, K, 1.0, As, M, Bs, K, 0.0, Cs, M))
-    out["zgemm_cn_4096_tflops"] = 8.0 * M * N * K / ms / 1e9
-    ms = timeit(lambda: torch.matmul(A, B))
-    out["cublas_zgemm_4096_tflops"] = 8.0 * M * N * K / ms / 1e9
-    # the S1 shapes: HER2K-lower K = 64+64 and HEMM m x 64
-    m = 16384
-    V, W = randc(m, 64, 3), randc(m, 64, 4)
-    Vs, Ws = cm(V), cm(W)
-    Cbig = torch.zeros((m, m), dtype=torch.complex128, device="cuda")
-    ms = timeit(lambda: eng.zgemm("N", "C", m, m, 64, -1.0, Vs, m, Ws, m, 1.0, Cbig, m, K2=64, A2=Ws, lda2=m,
-                                  B2=Vs, ldb2=m, lower_only=1), n=3)
-    out["her2k_lower_16384_k64_tflops"] = 8.0 * m * m * 64 / ms / 1e9
-    out["her2k_lower_16384_ms"] = ms
-    Xs = torch.zeros((64, m), dtype=torch.complex128, device="cuda")
-    for sk in (1, 2, 4):
-        ms = timeit(lambda: eng.zhemm_lower(m, 64, Cbig, m, Vs, m, Xs, m, splitk=sk), n=3)
-        out[f"hemm_lower_16384_splitk{sk}_tflops"] = 8.0 * m * m * 64 / ms / 1e9
-    Ar, Br = randr(M, K, 5), randr(K, N, 6)
-    Ars, Brs = cm(Ar), cm(Br)
-    Cr = torch.zeros((N, M), dtype=torch.float64, device="cuda")
-    ms = timeit(lambda: eng.dgemm(M, N, K, Ars, M, Brs, K, Cr, M))
-    out["dgemm_4096_tflops"] = 2.0 * M * N * K / ms / 1e9
-    ms = timeit(lambda: torch.matmul(Ar, Br))
-    out["cublas_dgemm_4096_tflops"] = 2.0 * M * N * K / ms / 1e9
-    os.makedirs("gpurun_out", exist_ok=True)
-    with open("gpurun_out/fp64_peak.json", "w") as f:
-        json.dump(out, f, indent=1)
-    print(json.dumps(out))
-    assert out["dmma_tflops_burst"] > 1.0
