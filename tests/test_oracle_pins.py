@@ -310,3 +310,47 @@ def test_sturm_count_matches_oracle_ql_on_random_tridiagonal():
     ok = gaps > 1e-8
     mids = (0.5 * (W[:-1] + W[1:]))[ok]
     assert np.array_equal(oracle.sturm_count(d, e, mids), (np.arange(1, n))[ok])
+
+
+# ---- pins for the rows widened in round 2 (the 1-stage and the real-symmetric variants).  The oracle for
+# both is O1-O5 itself (PAPER.md:148 steps i-iii executed naively; the real case is the same oracle on a real matrix).
+@pytest.mark.parametrize("n", [5, 40, 97])
+def test_tridiagonal_form_is_unique_up_to_phases(n):
+    """Implicit-Q theorem: with the first column of Q fixed to e_1, the Hermitian tridiagonal form of H has a unique
+    diagonal and unique |off-diagonals|.  LAPACK's Hessenberg reduction (scipy, a different code with a different
+    reflector convention) must therefore reproduce the oracle's d and e -- the element-wise reference the GPU's
+    eigh_tridiagonalise_direct is compared with."""
+    import scipy.linalg
+    rng = np.random.default_rng(300 + n)
+    A = rng.standard_normal((n, n)) + 1j * rng.standard_normal((n, n))
+    H = 0.5 * (A + A.conj().T)
+    d, e, Q = oracle.tridiagonalise(H)
+    Hs = scipy.linalg.hessenberg(H)
+    nrm = np.linalg.norm(H, 2)
+    assert np.abs(np.diag(Hs).real - d).max() <= 1e-11 * nrm
+    assert np.abs(np.abs(np.diag(Hs, -1)) - e).max() <= 1e-11 * nrm
+    assert np.abs(np.triu(Hs, 2)).max() <= 1e-12 * nrm           # Hermitian input: the Hessenberg form is tridiagonal
+
+
+def test_real_symmetric_input_gives_real_eigenvectors():
+    """The real-symmetric case of PAPER.md:140 / :158-160 is the same oracle on a real matrix: every step stays in the
+    reals (phi = +-1), so Z comes out exactly real and equals the textbook real decomposition; pinned on the closed form
+    of the 1-2-1 Toeplitz matrix embedded as a dense matrix and on config 0 (a real BdG matrix)."""
+    n = 64
+    T = 2.0 * np.eye(n) - np.eye(n, k=1) - np.eye(n, k=-1)
+    rng = np.random.default_rng(5)
+    Qr, _ = np.linalg.qr(rng.standard_normal((n, n)))
+    H = Qr @ T @ Qr.T
+    H = 0.5 * (H + H.T)
+    W, Z = oracle.eigh(H.astype(np.complex128))
+    assert np.abs(Z.imag).max() == 0.0
+    k = np.arange(1, n + 1)
+    assert np.abs(W - (2 - 2 * np.cos(k * np.pi / (n + 1)))).max() <= 1e-13
+    Zr = Z.real
+    assert np.abs(Zr.T @ Zr - np.eye(n)).max() <= 1e-13
+    assert np.linalg.norm(H @ Zr - Zr * W[None, :]) <= 1e-13 * n
+    H0 = wl.make_config(0).dense()
+    assert np.abs(H0.imag).max() == 0.0                         # config 0 is real-valued
+    p = wl.bdg_uniform((4, 4, 4), 0.5, 0.2)
+    W4, Z4 = oracle.eigh(p.dense())
+    assert np.abs(Z4.imag).max() == 0.0
