@@ -49,7 +49,13 @@ int eigh_create(eigh_handle_t* h, int64_t N, int64_t nev);
  * "hemm_waves" (S1.3: split-K of HEMM-lower sized for about this many thread blocks per SM; default 14),
  * "bt_chain" (S4a: consecutive passes of one column slab scheduled back to back so that followers read from L2;
  * 0 = automatic = 1, the unchained order), "bc_grid" (thread blocks of the S2 bulge-chasing kernel; 0 = every
- * co-resident block, the default), "band_width" (64: the only width S2 / S4a are built for; anything else is -3).
+ * co-resident block, the default), "band_width" (64: the only width S2 / S4a are built for; anything else is -3),
+ * "method" (2 = the two-stage solver, the default; 1 = the ONE-STAGE solver of PAPER.md:148 steps i-iii: direct
+ * blocked Householder tridiagonalisation, D&C, one back-transformation -- the solver the paper benchmarks in
+ * Figs. 3-4), "dtype" (0 = complex Hermitian c128, the default; 1 = REAL SYMMETRIC FP64:
+ * A_dev and Z_dev of eigh_solve / eigh_solve_host and of the *_direct entry points then hold `double` elements,
+ * lda / ldz in doubles; available for method = 1 only, so set "method" first), "ht_grid" (thread blocks of the
+ * 1-stage panel kernel; 0 = every co-resident block).
  * Changing an option invalidates the workspace: call eigh_workspace_size / eigh_set_workspace again afterwards
  * (every compute entry point returns -1 until then).  Returns -2 for an unknown key, -3 for a bad value. */
 int eigh_set_option(eigh_handle_t h, const char* key, int64_t value);
@@ -87,7 +93,8 @@ int eigh_solve_host(eigh_handle_t h, const void* A_host, int64_t lda, double* W_
 
 /* Per-phase device times of the last eigh_solve, in ms, from CUDA events on the solve's
  * stream: ms[0] = full->band, [1] = band->tridiagonal, [2] = tridiagonal D&C,
- * [3] = band back-transform, [4] = full back-transform. */
+ * [3] = band back-transform, [4] = full back-transform.  With method = 1: ms[0] = direct tridiagonalisation,
+ * [2] = D&C, [4] = back-transformation, [1] = [3] = 0. */
 int eigh_phase_times(eigh_handle_t h, double ms[5]);
 
 /* Device time (ms, CUDA events on the solve's stream around the launch) of one named kernel of the last
@@ -129,6 +136,21 @@ int eigh_band_to_tridiag(eigh_handle_t h, void* band_dev, int64_t ldab, double* 
  * Synchronises `stream`.  Returns the number of secular roots that failed to converge. */
 int eigh_tridiag_dc(eigh_handle_t h, const double* d_dev, const double* e_dev, double* W_dev,
                     double* Q_dev, int64_t ldq, void* stream);
+
+/* 1-stage variant, step i ("transforming the dense matrix into a tridiagonal form"; needs the option
+ * method = 1): unitary (orthogonal) Q = H_0 H_1 ... H_{N-2}, H_c = I - tau_c v_c v_c^H, with Q^H A Q = T real
+ * symmetric tridiagonal.  A_dev: N x N, c128 or (dtype = 1) double, lda >= N; only the LOWER triangle is read,
+ * imaginary parts of the diagonal are ignored; OVERWRITTEN: column c holds v_c in rows c+1.. (explicit unit element
+ * at row c+1).  d_dev[N] = diagonal of T; e_dev[N-1] = sub-diagonal (real, EITHER sign: eigh_tridiag_dc accepts it).
+ * The taus and the compact-WY T factors of the 64-column panels stay in the workspace for eigh_backtransform_direct.
+ * One persistent cooperative kernel per panel (HBM-bound: the lower triangle of the trailing matrix is read once per
+ * column, 8/3 N^3 bytes for c128, 4/3 N^3 for double) + one HER2K / SYR2K-lower GEMM per panel.  Enqueues on `stream`,
+ * does not synchronise. */
+int eigh_tridiagonalise_direct(eigh_handle_t h, void* A_dev, int64_t lda, double* d_dev, double* e_dev, void* stream);
+
+/* 1-stage variant, step iii: Z <- Q Z with the reflectors eigh_tridiagonalise_direct left in A_dev and the workspace.
+ * Z_dev: N x nev (c128 or double), ldz >= N, holds the eigenvectors of T on entry (as elements of the working type). */
+int eigh_backtransform_direct(eigh_handle_t h, const void* A_dev, int64_t lda, void* Z_dev, int64_t ldz, void* stream);
 
 /* Statistics of the last S3 run on this handle (eigh_tridiag_dc or eigh_solve), per merge level (level 0 = the
  * merges of pairs of leaves, the last level = the root merge):
@@ -220,6 +242,14 @@ int eigh_k_zgemm(eigh_handle_t h, char opA, char opB, int64_t M, int64_t N, int6
 int eigh_k_zhemm_lower(eigh_handle_t h, int64_t M, int64_t N, const void* A_dev, int64_t lda,
                        const void* B_dev, int64_t ldb, void* C_dev, int64_t ldc, int splitk,
                        void* stream);
+
+/* Real FP64 GEMM engine of the real-symmetric path (rgemm.cuh), same conventions as eigh_k_zgemm with op = 'N' or 'T':
+ *   C <- alpha * opA(A) * opB(B) [+ alpha * opA(A2) * opB(B2)] + beta * C,   lower_only bit 0 skips the 128 x 64 output
+ * tiles strictly above the diagonal (SYR2K-lower), splitk >= 1 = deterministic split-K. */
+int eigh_k_rgemm(eigh_handle_t h, char opA, char opB, int64_t M, int64_t N, int64_t K, double alpha, const double* A_dev,
+                 int64_t lda, const double* B_dev, int64_t ldb, int64_t K2, const double* A2_dev, int64_t lda2,
+                 const double* B2_dev, int64_t ldb2, double beta, double* C_dev, int64_t ldc, int lower_only, int splitk,
+                 void* stream);
 
 /* Real FP64 GEMM on the DMMA path: C (M x N) <- A[:, idx] * B, K inner; a_col_idx_dev may be
  * NULL (identity) or K int32 column indices into A. */

@@ -37,6 +37,8 @@ SIGNATURES = {
     "eigh_tridiag_dc": (_int, [_vp, _vp, _vp, _vp, _vp, _i64, _vp]),
     "eigh_backtransform_band": (_int, [_vp, _vp, _i64, _vp, _i64, _vp]),
     "eigh_backtransform_full": (_int, [_vp, _vp, _i64, _vp, _i64, _vp]),
+    "eigh_tridiagonalise_direct": (_int, [_vp, _vp, _i64, _vp, _vp, _vp]),
+    "eigh_backtransform_direct": (_int, [_vp, _vp, _i64, _vp, _i64, _vp]),
     "eigh_densities": (_int, [_vp, _vp, _vp, _i64, _i64, _dbl, _dbl, _int, _vp, _vp, _vp]),
     "eigh_gradient_densities": (_int, [_vp, _i64, _i64, _i64, _vp, _vp, _vp, _vp, _vp, _i64, _i64, _dbl, _dbl, _int,
                                        _vp, _vp, _vp]),
@@ -44,6 +46,8 @@ SIGNATURES = {
     "eigh_k_zgemm": (_int, [_vp, ctypes.c_char, ctypes.c_char, _i64, _i64, _i64, _dbl, _vp, _i64, _vp, _i64,
                             _i64, _vp, _i64, _vp, _i64, _dbl, _vp, _i64, _int, _int, _vp]),
     "eigh_k_zhemm_lower": (_int, [_vp, _i64, _i64, _vp, _i64, _vp, _i64, _vp, _i64, _int, _vp]),
+    "eigh_k_rgemm": (_int, [_vp, ctypes.c_char, ctypes.c_char, _i64, _i64, _i64, _dbl, _vp, _i64, _vp, _i64,
+                            _i64, _vp, _i64, _vp, _i64, _dbl, _vp, _i64, _int, _int, _vp]),
     "eigh_k_dgemm": (_int, [_vp, _i64, _i64, _i64, _vp, _i64, _vp, _vp, _i64, _vp, _i64, _vp]),
 }
 
@@ -132,11 +136,12 @@ class Eigh:
         is OVERWRITTEN.  Returns (W [N] float64, Zt [(nev, N)] complex128 with Zt[j] = eigenvector
         j, i.e. Z column-major).  Positive return codes (non-converged secular roots) raise."""
         import torch
-        assert At.is_cuda and At.dtype == torch.complex128 and At.is_contiguous() and At.shape == (self.N, self.N)
+        dt = self.dtype
+        assert At.is_cuda and At.dtype == dt and At.is_contiguous() and At.shape == (self.N, self.N)
         if W is None:
             W = torch.empty(self.N, dtype=torch.float64, device=At.device)
         if Zt is None:
-            Zt = torch.empty((self.nev, self.N), dtype=torch.complex128, device=At.device)
+            Zt = torch.empty((self.nev, self.N), dtype=dt, device=At.device)
         rc = self.lib.eigh_solve(self.h, _ptr(At), self.N, _ptr(W), _ptr(Zt), _stream())
         self._check(rc, "eigh_solve")
         return W, Zt
@@ -225,6 +230,27 @@ class Eigh:
         return int(self.lib.eigh_launch_count(self.h))
 
     # ------------------------------------------------------------------ phases
+    @property
+    def dtype(self):
+        """torch dtype of A and Z: complex128, or float64 with the option dtype = 1 (real symmetric, method = 1)."""
+        import torch
+        return torch.float64 if self.get_option("dtype") == 1 else torch.complex128
+
+    def tridiagonalise_direct(self, At, d, e):
+        """eigh_tridiagonalise_direct (1-stage, needs method = 1).  At: (N, N) storage of A column-major, overwritten."""
+        rc = self.lib.eigh_tridiagonalise_direct(self.h, _ptr(At), self.N, _ptr(d), _ptr(e), _stream())
+        self._check(rc, "eigh_tridiagonalise_direct")
+
+    def backtransform_direct(self, At, Zt):
+        rc = self.lib.eigh_backtransform_direct(self.h, _ptr(At), self.N, _ptr(Zt), Zt.shape[1], _stream())
+        self._check(rc, "eigh_backtransform_direct")
+
+    def rgemm(self, opA, opB, M, N, K, alpha, A, lda, B, ldb, beta, C, ldc, K2=0, A2=None, lda2=0, B2=None, ldb2=0,
+              lower_only=0, splitk=1):
+        rc = self.lib.eigh_k_rgemm(self.h, opA.encode(), opB.encode(), M, N, K, alpha, _ptr(A), lda, _ptr(B), ldb, K2,
+                                   _ptr(A2), lda2, _ptr(B2), ldb2, beta, _ptr(C), ldc, lower_only, splitk, _stream())
+        self._check(rc, "eigh_k_rgemm")
+
     def get_option(self, key: str) -> int:
         v = _i64()
         rc = self.lib.eigh_get_option(self.h, key.encode(), ctypes.byref(v))

@@ -11,6 +11,7 @@
 
 #include "dgemm.cuh"
 #include "eigh_internal.h"
+#include "rgemm.cuh"
 #include "zgemm.cuh"
 
 namespace eigh {
@@ -82,6 +83,8 @@ void plan_workspace(eigh_handle_s* h) {
         p.b4T = bump(off, (size_t)kb * kb * sizeof(c128));
         p.b4G = bump(off, (size_t)2 * kb * kb * sizeof(c128));
     }
+    p.ht_part = 0;
+    if (h->method == 1) p.ht_part = bump(off, ht_partial_bytes(N));
     p.total = off;
     h->planned = true;
 }
@@ -110,6 +113,8 @@ int eigh_create(eigh_handle_t* out, int64_t N, int64_t nev) {
     h->panel_smem = 1;
     h->panel_rows_min = 96;
     h->hemm_waves = 14;
+    h->method = 2;
+    h->real_dtype = 0;
     h->num_sms = 0;
     snprintf(h->err, sizeof(h->err), "ok");
     *out = h;
@@ -149,6 +154,17 @@ int eigh_set_option(eigh_handle_t h, const char* key, int64_t value) {
     } else if (!strcmp(key, "bc_grid")) {
         if (value < 0 || value > 4096) return set_err(h, -3, "bc_grid must be in [0, 4096]");
         h->bc_grid = (int)value;
+    } else if (!strcmp(key, "method")) {
+        if (value != 1 && value != 2) return set_err(h, -3, "method must be 1 (one-stage) or 2 (two-stage)");
+        if (value == 2 && h->real_dtype) return set_err(h, -3, "the real-symmetric path exists for method = 1 only");
+        h->method = (int)value;
+    } else if (!strcmp(key, "dtype")) {
+        if (value != 0 && value != 1) return set_err(h, -3, "dtype must be 0 (complex Hermitian, c128) or 1 (real symmetric, f64)");
+        if (value == 1 && h->method != 1) return set_err(h, -3, "dtype = 1 (real symmetric) needs method = 1: set \"method\" first");
+        h->real_dtype = (int)value;
+    } else if (!strcmp(key, "ht_grid")) {
+        if (value < 0 || value > 4096) return set_err(h, -3, "ht_grid must be in [0, 4096]");
+        h->ht_grid = (int)value;
     } else {
         return set_err(h, -2, "unknown option '%s'", key);
     }
@@ -174,6 +190,9 @@ int eigh_get_option(eigh_handle_t h, const char* key, int64_t* value) {
     else if (!strcmp(key, "bt_chain")) *value = h->bt_chain;
     else if (!strcmp(key, "hemm_waves")) *value = h->hemm_waves;
     else if (!strcmp(key, "bc_grid")) *value = h->bc_grid;
+    else if (!strcmp(key, "method")) *value = h->method;
+    else if (!strcmp(key, "dtype")) *value = h->real_dtype;
+    else if (!strcmp(key, "ht_grid")) *value = h->ht_grid;
     else return set_err(h, -2, "unknown option '%s'", key);
     return 0;
 }
@@ -236,6 +255,7 @@ static int cuda_fail(eigh_handle_t h, int rc, const char* where) {
 int eigh_reduce_to_band(eigh_handle_t h, void* A_dev, int64_t lda, void* band_dev, int64_t ldab, void* stream) {
     int rc = ensure_ready(h);
     if (rc) return rc;
+    if (h->method != 2) return set_err(h, -1, "eigh_reduce_to_band belongs to the two-stage method (option method = 2)");
     if (!A_dev) return -2;
     if (lda < h->N) return -3;
     if (!band_dev) return -4;
@@ -287,6 +307,28 @@ int eigh_backtransform_full(eigh_handle_t h, const void* A_dev, int64_t lda, voi
     if (!Z_dev) return -4;
     if (ldz < h->N) return -5;
     return cuda_fail(h, phase_backtransform_full(h, (const c128*)A_dev, lda, (c128*)Z_dev, ldz, (cudaStream_t)stream), "backtransform_full");
+}
+
+int eigh_tridiagonalise_direct(eigh_handle_t h, void* A_dev, int64_t lda, double* d_dev, double* e_dev, void* stream) {
+    int rc = ensure_ready(h);
+    if (rc) return rc;
+    if (h->method != 1) return set_err(h, -1, "eigh_tridiagonalise_direct needs the option method = 1");
+    if (!A_dev) return -2;
+    if (lda < h->N) return -3;
+    if (!d_dev) return -4;
+    if (!e_dev && h->N > 1) return -5;
+    return cuda_fail(h, phase_tridiagonalise_direct(h, A_dev, lda, d_dev, e_dev, (cudaStream_t)stream), "tridiagonalise_direct");
+}
+
+int eigh_backtransform_direct(eigh_handle_t h, const void* A_dev, int64_t lda, void* Z_dev, int64_t ldz, void* stream) {
+    int rc = ensure_ready(h);
+    if (rc) return rc;
+    if (h->method != 1) return set_err(h, -1, "eigh_backtransform_direct needs the option method = 1");
+    if (!A_dev) return -2;
+    if (lda < h->N) return -3;
+    if (!Z_dev) return -4;
+    if (ldz < h->N) return -5;
+    return cuda_fail(h, phase_backtransform_direct(h, A_dev, lda, nullptr, 0, Z_dev, ldz, (cudaStream_t)stream), "backtransform_direct");
 }
 
 int eigh_densities(eigh_handle_t h, const double* E_dev, const void* Z_dev, int64_t ldz, int64_t ncols, double T,
@@ -350,6 +392,37 @@ int eigh_solve(eigh_handle_t h, void* A_dev, int64_t lda, double* W_dev, void* Z
     const int64_t ldq = round_up(h->N, 8);
     h->launches = 0;
     int nfail = 0;
+    if (h->method == 1) {
+        // 1-stage variant (PAPER.md:148 steps i-iii): direct tridiagonalisation, D&C, one back-transformation.
+        // phase_ms: [0] = tridiagonalisation, [2] = D&C, [4] = back-transformation; [1] = [3] = 0.
+        NvtxRange whole1("eigh_solve (1-stage)");
+        cudaEventRecord(h->ev[0], s);
+        { NvtxRange r("1-stage tridiagonalisation");
+          rc = phase_tridiagonalise_direct(h, A_dev, lda, d, e, s); }
+        if (rc) return cuda_fail(h, rc, "tridiagonalise_direct");
+        cudaEventRecord(h->ev[1], s);
+        cudaEventRecord(h->ev[2], s);
+        { NvtxRange r("S3 tridiagonal D&C");
+          rc = phase_tridiag_dc(h, d, e, W_dev, Qt, ldq, s, &nfail); }
+        if (rc) return cuda_fail(h, rc, "tridiag_dc");
+        cudaEventRecord(h->ev[3], s);
+        cudaEventRecord(h->ev[4], s);
+        { NvtxRange r("1-stage back-transform");
+          rc = phase_backtransform_direct(h, A_dev, lda, Qt, ldq, Z_dev, h->N, s); }
+        if (rc) return cuda_fail(h, rc, "backtransform_direct");
+        cudaEventRecord(h->ev[5], s);
+        cudaError_t ce1 = cudaStreamSynchronize(s);
+        if (ce1 != cudaSuccess) return set_err(h, 1000 + (int)ce1, "eigh_solve: %s", cudaGetErrorString(ce1));
+        for (int i = 0; i < 5; ++i) {
+            float ms = 0.f;
+            cudaEventElapsedTime(&ms, h->ev[i], h->ev[i + 1]);
+            h->phase_ms[i] = ms;
+        }
+        h->phase_ms[1] = h->phase_ms[3] = 0.0;       // phases the 1-stage method does not have
+        h->sweep_ms = 0.0;
+        if (nfail) set_err(h, nfail, "%d secular roots did not converge", nfail);
+        return nfail;
+    }
     // NVTX ranges mark the host-side enqueue of every phase (the device-side spans are the CUDA events below)
     NvtxRange whole("eigh_solve");
     cudaEventRecord(h->ev[0], s);
@@ -619,6 +692,30 @@ int eigh_k_zhemm_lower(eigh_handle_t h, int64_t M, int64_t N, const void* A_dev,
         return set_err(h, -10, "splitk partials exceed workspace");
     rc = zgemm_launch(a, false, false, ZMODE_HEMM, true, (cudaStream_t)stream, &h->launches);
     return rc ? cuda_fail(h, 1000 + rc, "zhemm") : 0;
+}
+
+int eigh_k_rgemm(eigh_handle_t h, char opA, char opB, int64_t M, int64_t N, int64_t K, double alpha, const double* A_dev,
+                 int64_t lda, const double* B_dev, int64_t ldb, int64_t K2, const double* A2_dev, int64_t lda2,
+                 const double* B2_dev, int64_t ldb2, double beta, double* C_dev, int64_t ldc, int lower_only, int splitk,
+                 void* stream) {
+    int rc = ensure_ready(h);
+    if (rc) return rc;
+    const bool ta = (opA == 'T' || opA == 't'), tb = (opB == 'T' || opB == 't');
+    if (!ta && opA != 'N' && opA != 'n') return -2;
+    if (!tb && opB != 'N' && opB != 'n') return -3;
+    if (M < 0 || N < 0 || K < 0) return -4;
+    if (splitk < 1) return -20;
+    if (splitk > 1 && (size_t)splitk * M * N * sizeof(double) > h->plan.gemm_partial_bytes)
+        return set_err(h, -20, "splitk partials exceed workspace");
+    RgemmArgs a;
+    memset(&a, 0, sizeof(a));
+    a.M = (int)M; a.N = (int)N; a.K1 = (int)K; a.K2 = (int)K2;
+    a.A1 = A_dev; a.B1 = B_dev; a.lda1 = lda; a.ldb1 = ldb;
+    a.A2 = A2_dev; a.B2 = B2_dev; a.lda2 = lda2; a.ldb2 = ldb2;
+    a.C = C_dev; a.ldc = ldc; a.alpha = alpha; a.beta = beta; a.lower_only = lower_only & 1; a.splitk = splitk;
+    a.partial = ws_ptr<double>(h, h->plan.gemm_partial);
+    rc = rgemm_launch(a, ta, tb, (cudaStream_t)stream, &h->launches);
+    return rc ? cuda_fail(h, 1000 + rc, "rgemm") : 0;
 }
 
 int eigh_k_dgemm(eigh_handle_t h, int64_t M, int64_t N, int64_t K, const double* A_dev, int64_t lda,

@@ -460,6 +460,12 @@ int zgemm_ws(eigh_handle_s* h, bool ta, bool tb, int M, int N, int K, double alp
     return zg(h, ta, tb, M, N, K, alpha, A, lda, B, ldb, beta, C, ldc, small_tile, splitk, s);
 }
 
+int zgemm_ws2(eigh_handle_s* h, bool ta, bool tb, int M, int N, int K, double alpha, const c128* A, int64_t lda,
+              const c128* B, int64_t ldb, double beta, c128* C, int64_t ldc, bool small_tile, int splitk, cudaStream_t s,
+              int lower_only, int K2, const c128* A2, int64_t lda2, const c128* B2, int64_t ldb2) {
+    return zg(h, ta, tb, M, N, K, alpha, A, lda, B, ldb, beta, C, ldc, small_tile, splitk, s, lower_only, K2, A2, lda2, B2, ldb2);
+}
+
 static int splitk_for_small_output(int K) {
     int sk = K / 256;
     if (sk < 1) sk = 1;

@@ -32,6 +32,7 @@ struct WsPlan {
     size_t bt;                                 // back-transform scratch (S4b's Y, S4a's counters)
     size_t bt_bytes;
     size_t b4V, b4VT, b4Y, b4T, b4G;           // S4b merged-panel WY blocks: V, V T^H (N x kb), Y (kb x nev), T, G (kb x kb)
+    size_t ht_part;                            // 1-stage variant: per-tile partial products and per-row-block partials
     size_t total;
 };
 }  // namespace eigh
@@ -48,6 +49,9 @@ struct eigh_handle_s {
     int hemm_waves;      // S1.3: split-K of HEMM-lower chosen for about this many thread blocks per SM
     int bt_chain;   // S4a: consecutive passes of one slab scheduled back to back (0 = auto)
     int bc_grid;    // S2: CTAs of the bulge-chasing kernel (0 = all that are co-resident)
+    int method;     // 2 = two-stage (default), 1 = one-stage direct tridiagonalisation
+    int real_dtype; // 0 = complex Hermitian (c128), 1 = real symmetric (double); real needs method = 1
+    int ht_grid;    // 1-stage: thread blocks of the panel kernel (0 = all that are co-resident)
     int64_t ldab;   // band storage leading dimension
     void* ws;
     size_t ws_bytes;
@@ -107,6 +111,11 @@ int phase_backtransform_band(eigh_handle_s* h, const double* Q, int64_t ldq, c12
                              cudaStream_t s);
 int phase_backtransform_full(eigh_handle_s* h, const c128* A, int64_t lda, c128* Z, int64_t ldz,
                              cudaStream_t s);
+// 1-stage variant (tridiag_direct.cu); A / Z are c128 or double according to h->real_dtype
+int phase_tridiagonalise_direct(eigh_handle_s* h, void* A, int64_t lda, double* d, double* e, cudaStream_t s);
+int phase_backtransform_direct(eigh_handle_s* h, const void* A, int64_t lda, const double* Q, int64_t ldq, void* Z,
+                               int64_t ldz, cudaStream_t s);
+size_t ht_partial_bytes(int64_t N);
 // SCF epilogue (densities.cu): n(r), nu(r) of Eq. 16a / 16d from the columns of Z
 int launch_densities(eigh_handle_s* h, const double* E, const c128* Z, int64_t ldz, int64_t ncols, double T, double Ec,
                      int branch, double* n_out, c128* nu_out, cudaStream_t s);
