@@ -49,7 +49,9 @@ int eigh_create(eigh_handle_t* h, int64_t N, int64_t nev);
  * "hemm_waves" (S1.3: split-K of HEMM-lower sized for about this many thread blocks per SM; default 14),
  * "bt_chain" (S4a: consecutive passes of one column slab scheduled back to back so that followers read from L2;
  * 0 = automatic = 1, the unchained order), "bc_grid" (thread blocks of the S2 bulge-chasing kernel; 0 = every
- * co-resident block, the default), "band_width" (64: the only width S2 / S4a are built for; anything else is -3),
+ * co-resident block, the default), "bc_dual_steps" (S2: sweeps with at least this many chase steps run on the variant
+ * with two thread blocks per SM and no publisher warp; 0 = never, the default -- it measured 2-8 % slower at N = 27648 /
+ * 49152, the kernel being bound by L2 traffic rather than by occupancy), "band_width" (64: the only width S2 / S4a are built for; anything else is -3),
  * "method" (2 = the two-stage solver, the default; 1 = the ONE-STAGE solver of PAPER.md:148 steps i-iii: direct
  * blocked Householder tridiagonalisation, D&C, one back-transformation -- the solver the paper benchmarks in
  * Figs. 3-4), "dtype" (0 = complex Hermitian c128, the default; 1 = REAL SYMMETRIC FP64:

@@ -154,6 +154,9 @@ int eigh_set_option(eigh_handle_t h, const char* key, int64_t value) {
     } else if (!strcmp(key, "bc_grid")) {
         if (value < 0 || value > 4096) return set_err(h, -3, "bc_grid must be in [0, 4096]");
         h->bc_grid = (int)value;
+    } else if (!strcmp(key, "bc_dual_steps")) {
+        if (value < 0 || value > (1 << 20)) return set_err(h, -3, "bc_dual_steps must be in [0, 2^20]");
+        h->bc_dual_steps = (int)value;
     } else if (!strcmp(key, "method")) {
         if (value != 1 && value != 2) return set_err(h, -3, "method must be 1 (one-stage) or 2 (two-stage)");
         if (value == 2 && h->real_dtype) return set_err(h, -3, "the real-symmetric path exists for method = 1 only");
@@ -190,6 +193,7 @@ int eigh_get_option(eigh_handle_t h, const char* key, int64_t* value) {
     else if (!strcmp(key, "bt_chain")) *value = h->bt_chain;
     else if (!strcmp(key, "hemm_waves")) *value = h->hemm_waves;
     else if (!strcmp(key, "bc_grid")) *value = h->bc_grid;
+    else if (!strcmp(key, "bc_dual_steps")) *value = h->bc_dual_steps;
     else if (!strcmp(key, "method")) *value = h->method;
     else if (!strcmp(key, "dtype")) *value = h->real_dtype;
     else if (!strcmp(key, "ht_grid")) *value = h->ht_grid;

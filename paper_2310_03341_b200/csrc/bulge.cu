@@ -37,6 +37,7 @@ struct BcArgs {
     c128* tau2;       // [N][kmax]: tau of reflector (sweep j, step k) at tau2[j*kmax + k]
     int kmax;
     int* progress;    // [N], zero on entry
+    int j_begin, j_end;   // sweeps of this launch: j_begin <= j < j_end (sweep j_begin - 1, if any, is complete)
 };
 
 // Thread layout of one chase step: warp w owns rows 8w..8w+7 of a 64 x 64 block; lane = rl + 8 q
@@ -114,6 +115,7 @@ __device__ __forceinline__ void bc_handoff_wait(int odd) {
 struct BcStepCtx {
     c128* band; int64_t ldab;
     c128* Vj; c128* tau2j;
+    int* progress_j;             // progress counter of the current sweep (!PUB variant releases it itself)
     int r, q, rl, lane, warp, tid;
 };
 
@@ -139,7 +141,10 @@ __device__ __forceinline__ c128 bc_make_reflector(c128 x, const BcStepCtx& t, in
 
 // One chase step (sweep j, step k) by the compute group.  FULL: len = len2 = 64 (no edge predicates).
 // Returns false when the sweep ended with this step (no S block below).
-template <bool FULL>
+// PUB: a ninth (publisher) warp takes the release (one thread block per SM, 168 registers per thread); !PUB: thread 0 of the
+// compute group releases after a block barrier (two thread blocks of 8 warps per SM, 128 registers per thread: the second
+// block hides the latencies of the first -- used while the sweeps are long enough to keep 2 x 148 blocks busy).
+template <bool FULL, bool PUB>
 __device__ __forceinline__ bool bc_step(BcSmem& sm, const BcStepCtx& t, int r0, int len_, int len2_, int k, c128& tau, int& hb) {
     const int len = FULL ? BC_B : len_, len2 = FULL ? BC_B : len2_;
     const int r = t.r, q = t.q, rl = t.rl;
@@ -166,9 +171,14 @@ __device__ __forceinline__ bool bc_step(BcSmem& sm, const BcStepCtx& t, int r0, 
     }
     cp_async_wait<0>();
     bc_sync_compute();                                   // D landed; vs of this step visible
-    c128 vc[BC_NC];
+    // reflector entries of this thread's 16 columns: registers (PUB) or re-read from shared memory at every use (!PUB:
+    // 64 registers fewer; a quarter warp reads one address, i.e. a broadcast)
+    c128 vcreg[PUB ? BC_NC : 1];
+    if constexpr (PUB) {
 #pragma unroll
-    for (int i = 0; i < BC_NC; ++i) vc[i] = sm.vs[q + 4 * i];
+        for (int i = 0; i < BC_NC; ++i) vcreg[i] = sm.vs[q + 4 * i];
+    }
+    auto vc = [&](int i) -> c128 { if constexpr (PUB) return vcreg[i]; else return sm.vs[q + 4 * i]; };
     const c128 vr = sm.vs[r];
     // ---- the D phase (two-sided update of D_k) and the S phase (right update of S_{k+1}, next reflector) depend
     //      only on (v, tau): their matrix-vector products run in one loop, their block-wide reductions share one
@@ -187,8 +197,9 @@ __device__ __forceinline__ bool bc_step(BcSmem& sm, const BcStepCtx& t, int r0, 
                 e = sm.D[c <= r ? r + c * BC_LD : c + r * BC_LD];      // Hermitian D from its lower triangle
                 if (c >= r) e.y = (c == r) ? 0.0 : -e.y;
             }
-            cfma(accd[i & 3], e, vc[i]);
-            cfma(accs[i & 3], sreg[i], vc[i]);
+            const c128 vci = vc(i);
+            cfma(accd[i & 3], e, vci);
+            cfma(accs[i & 3], sreg[i], vci);
         }
         wr = cadd(cadd(accd[0], accd[1]), cadd(accd[2], accd[3]));
         ur = cadd(cadd(accs[0], accs[1]), cadd(accs[2], accs[3]));
@@ -202,8 +213,9 @@ __device__ __forceinline__ bool bc_step(BcSmem& sm, const BcStepCtx& t, int r0, 
         const c128 tu = cmul(tau, ur);
 #pragma unroll
         for (int i = 0; i < BC_NC; ++i) {
-            sreg[i].x -= tu.x * vc[i].x + tu.y * vc[i].y;
-            sreg[i].y -= tu.y * vc[i].x - tu.x * vc[i].y;
+            const c128 vci = vc(i);
+            sreg[i].x -= tu.x * vci.x + tu.y * vci.y;
+            sreg[i].y -= tu.y * vci.x - tu.x * vci.y;
         }
     }
     // partial sums of v^H (D v) and of the next reflector's norm (first column of S, held by the q = 0 lanes)
@@ -247,9 +259,10 @@ __device__ __forceinline__ bool bc_step(BcSmem& sm, const BcStepCtx& t, int r0, 
                 const int c = q + 4 * i;
                 if (c <= r) {
                     const c128 wc = sm.ws[c];
+                    const c128 vci = vc(i);
                     c128 e = sm.D[r + c * BC_LD];
-                    e.x -= pr.x * wc.x + pr.y * wc.y + qr.x * vc[i].x + qr.y * vc[i].y;
-                    e.y -= pr.y * wc.x - pr.x * wc.y + qr.y * vc[i].x - qr.x * vc[i].y;
+                    e.x -= pr.x * wc.x + pr.y * wc.y + qr.x * vci.x + qr.y * vci.y;
+                    e.y -= pr.y * wc.x - pr.x * wc.y + qr.y * vci.x - qr.x * vci.y;
                     if (c == r) e.y = 0.0;
                     dp[(int64_t)i * 4 * (ldab - 1)] = e;
                 }
@@ -261,16 +274,28 @@ __device__ __forceinline__ bool bc_step(BcSmem& sm, const BcStepCtx& t, int r0, 
     //      release of "step k" is handed to the publisher warp now, and the rest of the step (left update of S_{k+1}, its
     //      stores, the reflector) runs behind it: the lag between consecutive sweeps drops from 2 steps to ~1.6.
     if (has_s && r == 0 && q == 0) band[BC_B + (int64_t)r0 * ldab] = cmake(betan, 0.0);
-    bc_handoff_arrive(hb);
-    hb ^= 1;
+    if constexpr (PUB) {
+        bc_handoff_arrive(hb);
+        hb ^= 1;
+    } else {
+        bc_sync_compute();                                   // every thread's stores of this step are issued
+        if (t.tid == 0) bc_st_release(t.progress_j, has_s ? k + 1 : INT_MAX);
+    }
     if (!has_s) return false;
     // ---- z_c = vn^H S[:, c]: per-thread products, reduce-scatter over the 8 row lanes, then across warps
     {
-        c128 zp[BC_NC];
+        // (the first exchange is folded into the products: 8 partial sums are live instead of 16)
+        c128 zp[BC_NC / 2];
+        {
+            const bool up0 = rl & 1;
 #pragma unroll
-        for (int i = 0; i < BC_NC; ++i) zp[i] = cmulc(vnr, sreg[i]);
+            for (int i = 0; i < BC_NC / 2; ++i) {
+                const c128 a0 = cmulc(vnr, sreg[i]), a1 = cmulc(vnr, sreg[i + BC_NC / 2]);
+                zp[i] = cadd(up0 ? a1 : a0, bc_shfl_xor(up0 ? a0 : a1, 1));
+            }
+        }
 #pragma unroll
-        for (int st = 0; st < 3; ++st) {
+        for (int st = 1; st < 3; ++st) {
             const int half = BC_NC >> (st + 1);
             const bool up = (rl >> st) & 1;
 #pragma unroll
@@ -320,18 +345,19 @@ __device__ __forceinline__ bool bc_step(BcSmem& sm, const BcStepCtx& t, int r0, 
     return true;
 }
 
-__global__ void __launch_bounds__(BC_NT + 32, 1) bulge_chase_kernel(const BcArgs a) {
+template <bool PUB>
+__global__ void __launch_bounds__(PUB ? BC_NT + 32 : BC_NT, PUB ? 1 : 2) bulge_chase_kernel(const BcArgs a) {
     extern __shared__ __align__(16) unsigned char bc_raw[];
     BcSmem& sm = *reinterpret_cast<BcSmem*>(bc_raw);
 
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int N = a.N;
 
-    if (warp == BC_NW) {
+    if (PUB && warp == BC_NW) {
         // ================= publisher warp: one release per step whose D phase is complete (the previous step is then
         // complete in full), INT_MAX per completed sweep
         int hb = 0;
-        for (int j = blockIdx.x; j <= N - 2; j += gridDim.x) {
+        for (int j = a.j_begin + blockIdx.x; j < a.j_end; j += gridDim.x) {
             for (int k = 0;; ++k) {
                 const bool more = N - (j + 1 + k * BC_B + BC_B) > 0;
                 bc_handoff_wait(hb);
@@ -350,9 +376,10 @@ __global__ void __launch_bounds__(BC_NT + 32, 1) bulge_chase_kernel(const BcArgs
     const int r = t.r, q = t.q;
     int hb = 0;
 
-    for (int j = blockIdx.x; j <= N - 2; j += gridDim.x) {
+    for (int j = a.j_begin + blockIdx.x; j < a.j_end; j += gridDim.x) {
         t.Vj = a.V2 + ((a.pass_off[j >> 5] * 32 + (j & 31)) * BC_B);     // reflector (j, k) at Vj[k * 2048 + i]
         t.tau2j = a.tau2 + (int64_t)j * a.kmax;
+        t.progress_j = a.progress + j;
         if (tid == 0) bc_poll(a.progress, j - 1, 2);
         bc_sync_compute();
         // ---- reflector (j, 0) from column j of the band
@@ -378,8 +405,8 @@ __global__ void __launch_bounds__(BC_NT + 32, 1) bulge_chase_kernel(const BcArgs
             const int len = min(BC_B, N - r0);
             const int len2 = min(BC_B, N - (r0 + BC_B));
             // (the release of the step is handed to the publisher warp inside bc_step, after the D phase)
-            const bool more = (len == BC_B && len2 == BC_B) ? bc_step<true>(sm, t, r0, len, len2, k, tau, hb)
-                                                            : bc_step<false>(sm, t, r0, len, len2, k, tau, hb);
+            const bool more = (len == BC_B && len2 == BC_B) ? bc_step<true, PUB>(sm, t, r0, len, len2, k, tau, hb)
+                                                            : bc_step<false, PUB>(sm, t, r0, len, len2, k, tau, hb);
             if (!more) break;
             if (tid == 0) bc_poll(a.progress, j - 1, k + 3);
             bc_sync_compute();
@@ -418,20 +445,47 @@ int phase_band_to_tridiag(eigh_handle_s* h, c128* band, int64_t ldab, double* d,
     }
     if (N >= 2) {
         const size_t smem = sizeof(BcSmem);
-        EIGH_CUDA_OK(cudaFuncSetAttribute(bulge_chase_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        int occ = 0;
-        EIGH_CUDA_OK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, bulge_chase_kernel, BC_NT + 32, smem));
-        if (occ < 1) return set_err(h, EIGH_ERR_CUDA, "bulge_chase_kernel cannot be resident");
-        int G = h->num_sms * occ;
-        if (h->bc_grid > 0 && h->bc_grid < G) G = h->bc_grid;
-        if (G > N - 1) G = N - 1;
         BcArgs a;
         a.band = band; a.ldab = ldab; a.N = N; a.V2 = ws_ptr<c128>(h, pl.V2); a.progress = progress;
         a.pass_off = ws_ptr<int64_t>(h, pl.pass_off);
         a.tau2 = ws_ptr<c128>(h, pl.tau2); a.kmax = (int)bc_kmax(h);
+        // Long sweeps first, with TWO thread blocks per SM (no publisher warp, 128 registers): while a sweep has more than
+        // ~2 x (2 x 148) steps every block is busy and the second block of an SM hides the latencies of the first.  The
+        // remaining sweeps run with one block per SM (publisher warp, 168 registers), whose single step is faster: there the
+        // lag between consecutive sweeps, not the number of blocks, bounds the rate.
+        int j_switch = 0;
+        if (h->bc_dual_steps > 0) {
+            const int64_t js = (int64_t)N - 1 - (int64_t)h->bc_dual_steps * BC_B;
+            j_switch = js > 0 ? (int)js : 0;
+            if (j_switch > N - 1) j_switch = N - 1;
+        }
         void* kargs[] = {(void*)&a};
-        EIGH_CUDA_OK(cudaLaunchCooperativeKernel((void*)bulge_chase_kernel, dim3(G), dim3(BC_NT + 32), kargs, smem, s));
-        ++h->launches;
+        if (j_switch > 0) {
+            auto kern = bulge_chase_kernel<false>;
+            EIGH_CUDA_OK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+            int occ = 0;
+            EIGH_CUDA_OK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kern, BC_NT, smem));
+            if (occ < 1) return set_err(h, EIGH_ERR_CUDA, "bulge_chase_kernel<dual> cannot be resident");
+            int G = h->num_sms * occ;
+            if (h->bc_grid > 0 && h->bc_grid < G) G = h->bc_grid;
+            if (G > j_switch) G = j_switch;
+            a.j_begin = 0; a.j_end = j_switch;
+            EIGH_CUDA_OK(cudaLaunchCooperativeKernel((void*)kern, dim3(G), dim3(BC_NT), kargs, smem, s));
+            ++h->launches;
+        }
+        if (j_switch < N - 1) {
+            auto kern = bulge_chase_kernel<true>;
+            EIGH_CUDA_OK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+            int occ = 0;
+            EIGH_CUDA_OK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kern, BC_NT + 32, smem));
+            if (occ < 1) return set_err(h, EIGH_ERR_CUDA, "bulge_chase_kernel cannot be resident");
+            int G = h->num_sms * occ;
+            if (h->bc_grid > 0 && h->bc_grid < G) G = h->bc_grid;
+            if (G > N - 1 - j_switch) G = N - 1 - j_switch;
+            a.j_begin = j_switch; a.j_end = N - 1;
+            EIGH_CUDA_OK(cudaLaunchCooperativeKernel((void*)kern, dim3(G), dim3(BC_NT + 32), kargs, smem, s));
+            ++h->launches;
+        }
     }
     extract_tridiag_kernel<<<(unsigned)ceil_div(N, 256), 256, 0, s>>>(band, ldab, N, d, e, sgn);
     ++h->launches;

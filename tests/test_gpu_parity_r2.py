@@ -142,6 +142,8 @@ _OPTION_CASES = [
     ({"hemm_waves": 1}, 2100),
     ({"hemm_waves": 40}, 2100),
     ({"bc_grid": 7}, 2100),
+    ({"bc_dual_steps": 1}, 2100),        # every sweep on the two-blocks-per-SM kernel
+    ({"bc_dual_steps": 20}, 2100),       # long sweeps on the dual kernel, the rest on the publisher kernel
 ]
 
 
