@@ -244,6 +244,11 @@ def main():
                     help="also time library routines on the same matrix as CONTEXT (never the target, never on the hot path): "
                          "torch.linalg.eigh (cuSOLVER) on this GPU and numpy.linalg.eigh (LAPACK) on the CPU sample")
     ap.add_argument("--opt", action="append", default=[], help="solver option key=value (eigh_set_option), repeatable")
+    ap.add_argument("--method", type=int, default=2, choices=(1, 2),
+                    help="2 = two-stage solver (the hot path, default); 1 = the 1-stage variant of SURVEY.md 8(f)2 "
+                         "(PAPER.md:148 steps i-iii; use with --config 0..2)")
+    ap.add_argument("--real", action="store_true",
+                    help="real-symmetric FP64 path (needs --method 1 and a real matrix: --config 0)")
     args = ap.parse_args()
     # W >= 3 is the timing rule for a valid bench number; smaller values are accepted for profiler runs only
     # (ncu launch lists), whose printed numbers are never bench values
@@ -273,18 +278,29 @@ def main():
     N = w.N
     nev, nev_rule = choose_nev(args.config, N, w.nev_runs, args.warmup, args.steps, args.time_budget, args.nev)
     opts = {}
+    if args.method == 1:
+        opts["method"] = 1
+        if args.real:
+            opts["dtype"] = 1
     for kv in args.opt:
         key, val = kv.split("=")
         opts[key] = int(val)
     solver = binding.Eigh(N, nev, device=dev, **opts)
     b = solver.band_width                                    # read from the handle (eigh_get_option)
     mat_bytes = N * N * 16
-    At = torch.empty((N, N), dtype=torch.complex128, device=dev)       # A column-major (stored as A^T row-major)
+    wdt = solver.dtype                                       # complex128, or float64 on the real-symmetric path
+    At = torch.empty((N, N), dtype=wdt, device=dev)          # A column-major (stored as A^T row-major)
     W = torch.empty(N, dtype=torch.float64, device=dev)
-    Zt = torch.empty((nev, N), dtype=torch.complex128, device=dev)
+    Zt = torch.empty((nev, N), dtype=wdt, device=dev)
     pristine = None
     fields = None
-    if w.problem is not None:
+    if args.real:
+        tmp = torch.empty((N, N), dtype=torch.complex128, device=dev)
+        w.dense_torch(dev, out=tmp)
+        assert float(tmp.imag.abs().max().item()) == 0.0, "--real needs a real matrix (config 0)"
+        pristine = tmp.real.contiguous()
+        del tmp
+    elif w.problem is not None:
         # BdG configs: H is re-assembled on the device from its fields by the library's own prologue kernel
         pb = w.problem
         fields = ([torch.from_numpy(wl_mod.kinetic_1d(L)).to(dev) for L in pb.shape],
@@ -346,9 +362,11 @@ def main():
         with torch.no_grad():
             regenerate()
             Hl = At.t()                                          # logical H (all N^2 elements are valid)
+            if args.real:
+                Hl = Hl.to(torch.complex128)
             ncheck = min(nev, 256)
             cols = torch.linspace(0, nev - 1, ncheck, device=dev).long()
-            Zc = Zt[cols].t()                                   # N x ncheck
+            Zc = Zt[cols].t().to(torch.complex128)              # N x ncheck
             R = Hl @ Zc - Zc * W[cols][None, :]
             hn = float(torch.linalg.norm(Hl).item())
             valid["residual_sampled"] = float(torch.linalg.norm(R).item()) / (hn * (ncheck ** 0.5))
@@ -368,7 +386,7 @@ def main():
     # Eq. 16a/16d at T = 0.  HBM-bound: algorithmic bytes = the u and v halves of every ACTIVE column of Z read once
     # (16 N bytes per column) + the two output fields; CUDA events on the launching stream.
     epilogue = None
-    if rank == 0 and w.problem is not None and N % 2 == 0 and not args.no_epilogue:
+    if rank == 0 and w.problem is not None and N % 2 == 0 and not args.no_epilogue and not args.real:
         try:
             branch = 1 if nev == N else -1                       # lowest N/2 pairs: particle-hole partners (reading 3)
             E = W[:nev].contiguous()
@@ -433,10 +451,10 @@ def main():
         try:
             regenerate()
             torch.cuda.synchronize()
-            Ah = torch.empty((N, N), dtype=torch.complex128)
+            Ah = torch.empty((N, N), dtype=wdt)
             Ah.copy_(At)
             Wh = torch.empty(N, dtype=torch.float64)
-            Zh = torch.empty((nev, N), dtype=torch.complex128)
+            Zh = torch.empty((nev, N), dtype=wdt)
             times = []
             for i in range(2 if N <= 8192 else 1):
                 torch.cuda.synchronize()
@@ -445,7 +463,7 @@ def main():
                 torch.cuda.synchronize()
                 times.append(time.perf_counter() - tt)
             e2e = {"value": min(times), "unit": "s", "h2d_bytes_per_step": mat_bytes,
-                   "d2h_bytes_per_step": N * 8 + N * nev * 16,
+                   "d2h_bytes_per_step": N * 8 + N * nev * (8 if args.real else 16),
                    "host_buffers": "pageable, streamed through a 2 x 256 MiB pinned ring (eigh_solve_host)",
                    "check_W_max_abs_diff": float((Wh - W.cpu()).abs().max().item())}
             del Ah, Zh
@@ -558,14 +576,42 @@ def main():
         "p2_hbm_frac_credited": (cw["p2_bytes"] / ph[1] / 1e6) / hbm if ph[1] and hbm else None,
     }
     cfg = config_dict(w, nev, nev_rule, b)
+    if args.method == 1:
+        # 1-stage variant.  Dominant kernel = hetrd_panel_kernel (one cooperative launch per 64-column
+        # panel, all inside phase 0 together with the HER2K / SYR2K GEMMs): HBM-bound, algorithmic bytes = the lower
+        # triangle of the trailing matrix read once per column, sum_c es (N-1-c)(N-c)/2  (~ es N^3 / 6; es = 16 or 8).
+        es = 8 if args.real else 16
+        tri_bytes = float(sum(es * (N - 1 - c) * (N - c) // 2 for c in range(N - 1)))
+        npanels = -(-(N - 1) // 64)
+        bt_flops = (2.0 if args.real else 8.0) * N * N * nev
+        upd_flops = (2.0 if args.real else 8.0) * N ** 3 / 3.0          # rank-2k updates (HER2K-lower)
+        phase_report = {
+            "p1_tridiagonalise_direct": {"ms": ph[0], "gbs_lower_triangle": tri_bytes / ph[0] / 1e6 if ph[0] else None,
+                                         "her2k_flops": upd_flops, "panels": npanels},
+            "p3_tridiag_dc": phase_report["p3_tridiag_dc"],
+            "p4_backtransform_direct": {"ms": ph[4], "tflops": tf(bt_flops, ph[4])},
+        }
+        ach = tri_bytes / ph[0] / 1e6 if ph[0] else 0.0
+        roofline = {
+            "bound": "hbm", "kernel": "eigh::hetrd_panel_kernel<%s> (%d cooperative launches per solve, phase p1; the phase "
+                                      "time also holds the %d rank-2k GEMM updates)" % ("double" if args.real else "c128", npanels, npanels),
+            "achieved": ach, "peak": hbm, "unit": "GB/s", "frac": ach / hbm if hbm else None, "traffic": None,
+            "traffic_source": "no ncu capture", "algorithmic_bytes_per_step": tri_bytes,
+            "algorithmic_bytes_per_launch": tri_bytes / npanels, "kernel_ms": ph[0] / npanels, "launches_per_step": npanels,
+            "kernel_share_of_step": ph[0] / ms_per_step if ms_per_step else None,
+            "peak_source": "MEASURED_PEAKS.json hbm_gbs (of measured); for N below ~4000 the lower triangle fits the 126 MB L2",
+        }
+        cfg["method"] = "one-stage (PAPER.md:148 steps i-iii)"
+        cfg["dtype"] = "f64 real symmetric" if args.real else "c128"
     line = {
         "metric": "eigh_time_s", "value": value_s, "unit": "s", "n_gpus": world, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": ms_per_step, "higher_is_better": False, "scaling": "weak",
-        "vs_baseline": None, "dtype": "c128", "data": "synthetic",
+        "vs_baseline": None, "dtype": "f64" if args.real else "c128", "data": "synthetic",
         "config": cfg,
         "clocks": clocks, "e2e": e2e, "gpu_launches": launches, "phases": phase_report, "roofline": roofline,
         "cpu_baseline": cpu, "validity": valid, "epilogue": epilogue, "context": context,
-        "total_tflops": (cw["p1_flops"] + cw["p2_flops"] + cw["p4a_flops"] + cw["p4b_flops"]) / ms_per_step / 1e9,
+        "total_tflops": (cw["p1_flops"] + cw["p2_flops"] + cw["p4a_flops"] + cw["p4b_flops"]) / ms_per_step / 1e9
+        if args.method == 2 else None,
     }
     print(json.dumps(line))
     if dist is not None:

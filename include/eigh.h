@@ -224,6 +224,40 @@ int eigh_assemble_bdg(eigh_handle_t h, int64_t nx, int64_t ny, int64_t nz, const
                       double mu, double sign, void* A_dev, int64_t lda, void* stream);
 
 /* ---------------------------------------------------------------------------------------
+ * Second workload: one TDSLDA time step for the states just computed.
+ * PAPER.md:91 Eq. (5):  i d/dt [u_n, v_n]^T = [[h, Delta], [Delta^*, -h^*]] [u_n, v_n]^T  (hbar = 1), h = -1/2 lap + V - mu
+ * with the spectral kinetic term of Eq. (8) in its matrix form: one dense real symmetric 1-D matrix
+ * per axis (the Kx, Ky, Kz of eigh_assemble_bdg), applied on the FP64 tensor cores.  States are columns of an N x ncols
+ * c128 array (rows [0, M) = u, [M, 2M) = v, grid point r = (ix ny + iy) nz + iz, M = nx ny nz = N/2).
+ * ------------------------------------------------------------------------------------- */
+
+/* F <- -i H(V, Delta) Phi, the right-hand side of Eq. (5) for ncols states.  V_dev: M doubles; Delta_dev: M c128;
+ * Phi_dev: N x ncols c128, ldp >= N (read only); F_dev: N x ncols c128, ldf >= N (out; must not alias Phi_dev).
+ * Three launches (one per axis; the last fuses the local terms and the factor -i); HBM-bound, 8 x 16 N bytes per state.
+ * Uses the handle's N only (no workspace contents); enqueues on `stream`, does not synchronise. */
+int eigh_tdslda_rhs(eigh_handle_t h, int64_t nx, int64_t ny, int64_t nz, const double* Kx_dev, const double* Ky_dev,
+                    const double* Kz_dev, const double* V_dev, const void* Delta_dev, double mu, const void* Phi_dev,
+                    int64_t ldp, int64_t ncols, void* F_dev, int64_t ldf, void* stream);
+
+/* One step y_n -> y_{n+1} of the 5th-order Adams-Bashforth-Moulton predictor-corrector of PAPER.md:134 in PECE form
+ * (the paper names the method only; the coefficients are the textbook 5-step Adams-Bashforth predictor and 4-step
+ * Adams-Moulton corrector), with h and Delta evaluated twice, each time from the densities of the current states
+ * (eigh_densities: Eq. 16a / 16d with the occupation weights of the INITIAL energies E0_dev, T, Ec, branch) through the
+ * toy functional Delta(r) = g nu(r) (Eq. 18b with a constant coupling; V stays fixed):
+ *     y_p     = y_n + dt/720 (1901 f_n - 2774 f_{n-1} + 2616 f_{n-2} - 1274 f_{n-3} + 251 f_{n-4}),   f_p = -i H[y_p] y_p
+ *     y_{n+1} = y_n + dt/720 (251 f_p + 646 f_n - 264 f_{n-1} + 106 f_{n-2} - 19 f_{n-3}),           f_{n+1} = -i H[y_{n+1}] y_{n+1}
+ *   Y_dev    : N x ncols c128, ldy >= N: y_n on entry, y_{n+1} on return.
+ *   F_dev    : HOST array of 5 device pointers, F_dev[k] = f_{n-k} (N x ncols c128 each, ldf >= N).  On return the
+ *              buffer F_dev[4] holds f_{n+1}; the others are unchanged: rotate to [F4, F0, F1, F2, F3] for the next step.
+ *   Yp_dev   : N x ncols c128 scratch (ld = ldy) for the predicted state.   7 copies of the state in all.
+ *   n_dev    : M doubles (out): n(r) of y_{n+1}.   Delta_dev : M c128 (out): g nu(r) of y_{n+1}.
+ * Uses the handle's workspace (the densities); 20 launches on `stream`, does not synchronise. */
+int eigh_tdslda_step(eigh_handle_t h, int64_t nx, int64_t ny, int64_t nz, const double* Kx_dev, const double* Ky_dev,
+                     const double* Kz_dev, const double* V_dev, double g, double mu, const double* E0_dev, double T, double Ec,
+                     int branch, double dt, void* Y_dev, int64_t ldy, void* const F_dev[5], int64_t ldf, void* Yp_dev,
+                     int64_t ncols, double* n_dev, void* Delta_dev, void* stream);
+
+/* ---------------------------------------------------------------------------------------
  * Kernel-level entry points (unit tests of the building blocks).
  * ------------------------------------------------------------------------------------- */
 

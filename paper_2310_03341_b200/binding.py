@@ -43,6 +43,9 @@ SIGNATURES = {
     "eigh_gradient_densities": (_int, [_vp, _i64, _i64, _i64, _vp, _vp, _vp, _vp, _vp, _i64, _i64, _dbl, _dbl, _int,
                                        _vp, _vp, _vp]),
     "eigh_assemble_bdg": (_int, [_vp, _i64, _i64, _i64, _vp, _vp, _vp, _vp, _vp, _dbl, _dbl, _vp, _i64, _vp]),
+    "eigh_tdslda_rhs": (_int, [_vp, _i64, _i64, _i64, _vp, _vp, _vp, _vp, _vp, _dbl, _vp, _i64, _i64, _vp, _i64, _vp]),
+    "eigh_tdslda_step": (_int, [_vp, _i64, _i64, _i64, _vp, _vp, _vp, _vp, _dbl, _dbl, _vp, _dbl, _dbl, _int, _dbl, _vp,
+                                _i64, ctypes.POINTER(_vp), _i64, _vp, _i64, _vp, _vp, _vp]),
     "eigh_k_zgemm": (_int, [_vp, ctypes.c_char, ctypes.c_char, _i64, _i64, _i64, _dbl, _vp, _i64, _vp, _i64,
                             _i64, _vp, _i64, _vp, _i64, _dbl, _vp, _i64, _int, _int, _vp]),
     "eigh_k_zhemm_lower": (_int, [_vp, _i64, _i64, _vp, _i64, _vp, _i64, _vp, _i64, _int, _vp]),
@@ -214,6 +217,33 @@ class Eigh:
                                         float(mu), float(sign), _ptr(At), self.N, _stream())
         self._check(rc, "eigh_assemble_bdg")
         return At
+
+    # ------------------------------------------------------------------ second workload: TDSLDA step
+    def tdslda_rhs(self, shape, Kx, Ky, Kz, V, Delta, mu, Phit, Ft=None):
+        """eigh_tdslda_rhs: Ft <- -i H Phi.  Phit, Ft: (ncols, N) complex128 (states = rows, i.e. column-major N x ncols)."""
+        import torch
+        nx, ny, nz = (int(v) for v in shape)
+        if Ft is None:
+            Ft = torch.empty_like(Phit)
+        rc = self.lib.eigh_tdslda_rhs(self.h, nx, ny, nz, _ptr(Kx), _ptr(Ky), _ptr(Kz), _ptr(V), _ptr(Delta), float(mu),
+                                      _ptr(Phit), int(Phit.stride(0)) if Phit.shape[0] > 1 else self.N, int(Phit.shape[0]),
+                                      _ptr(Ft), int(Ft.stride(0)) if Ft.shape[0] > 1 else self.N, _stream())
+        self._check(rc, "eigh_tdslda_rhs")
+        return Ft
+
+    def tdslda_step(self, shape, Kx, Ky, Kz, V, g, mu, E0, dt, Yt, Flist, Ypt, n, Delta, T=0.0, Ec=float("inf"), branch=1):
+        """eigh_tdslda_step.  Yt, Ypt and the five tensors of Flist ([f_n, ..., f_{n-4}]): (ncols, N) complex128 contiguous.
+        Returns the rotated list [f_{n+1}, f_n, ..., f_{n-3}] (same tensors, no copy)."""
+        nx, ny, nz = (int(v) for v in shape)
+        ncols = int(Yt.shape[0])
+        for t in [Yt, Ypt] + list(Flist):
+            assert t.is_cuda and t.is_contiguous() and t.shape == (ncols, self.N)
+        arr = (_vp * 5)(*[t.data_ptr() for t in Flist])
+        rc = self.lib.eigh_tdslda_step(self.h, nx, ny, nz, _ptr(Kx), _ptr(Ky), _ptr(Kz), _ptr(V), float(g), float(mu), _ptr(E0),
+                                       float(T), float(Ec), int(branch), float(dt), _ptr(Yt), self.N, arr, self.N, _ptr(Ypt),
+                                       ncols, _ptr(n), _ptr(Delta), _stream())
+        self._check(rc, "eigh_tdslda_step")
+        return [Flist[4]] + list(Flist[:4])
 
     def phase_times_ms(self):
         ms = (ctypes.c_double * 5)()

@@ -313,6 +313,70 @@ int eigh_backtransform_full(eigh_handle_t h, const void* A_dev, int64_t lda, voi
     return cuda_fail(h, phase_backtransform_full(h, (const c128*)A_dev, lda, (c128*)Z_dev, ldz, (cudaStream_t)stream), "backtransform_full");
 }
 
+static int grid_check(eigh_handle_t h, int64_t nx, int64_t ny, int64_t nz, const char* who) {
+    if (h->N & 1) return set_err(h, -1, "%s: N = %lld is odd (phi = [u, v] needs N = 2M)", who, (long long)h->N);
+    if (nx < 1 || ny < 1 || nz < 1 || nx > 64 || ny > 64 || nz > 64) return set_err(h, -2, "%s: grid extents must be 1..64 per axis", who);
+    if (2 * nx * ny * nz != h->N)
+        return set_err(h, -2, "%s: 2 nx ny nz = %lld != N = %lld", who, (long long)(2 * nx * ny * nz), (long long)h->N);
+    return 0;
+}
+
+int eigh_tdslda_rhs(eigh_handle_t h, int64_t nx, int64_t ny, int64_t nz, const double* Kx_dev, const double* Ky_dev,
+                    const double* Kz_dev, const double* V_dev, const void* Delta_dev, double mu, const void* Phi_dev,
+                    int64_t ldp, int64_t ncols, void* F_dev, int64_t ldf, void* stream) {
+    int rc = ensure_ready(h);
+    if (rc) return rc;
+    rc = grid_check(h, nx, ny, nz, "eigh_tdslda_rhs");
+    if (rc) return rc;
+    if (!Kx_dev) return -5;
+    if (!Ky_dev) return -6;
+    if (!Kz_dev) return -7;
+    if (!V_dev) return -8;
+    if (!Delta_dev) return -9;
+    if (!Phi_dev && ncols > 0) return -11;
+    if (ldp < h->N) return -12;
+    if (ncols < 0) return -13;
+    if (!F_dev && ncols > 0) return -14;
+    if (ldf < h->N) return -15;
+    if (F_dev == Phi_dev && ncols > 0) return set_err(h, -14, "eigh_tdslda_rhs: F must not alias Phi");
+    return cuda_fail(h, launch_tdslda_rhs(h, (int)nx, (int)ny, (int)nz, Kx_dev, Ky_dev, Kz_dev, V_dev, (const c128*)Delta_dev, mu,
+                                          (const c128*)Phi_dev, ldp, ncols, (c128*)F_dev, ldf, (cudaStream_t)stream), "tdslda_rhs");
+}
+
+int eigh_tdslda_step(eigh_handle_t h, int64_t nx, int64_t ny, int64_t nz, const double* Kx_dev, const double* Ky_dev,
+                     const double* Kz_dev, const double* V_dev, double g, double mu, const double* E0_dev, double T, double Ec,
+                     int branch, double dt, void* Y_dev, int64_t ldy, void* const F_dev[5], int64_t ldf, void* Yp_dev,
+                     int64_t ncols, double* n_dev, void* Delta_dev, void* stream) {
+    int rc = ensure_ready(h);
+    if (rc) return rc;
+    rc = grid_check(h, nx, ny, nz, "eigh_tdslda_step");
+    if (rc) return rc;
+    if (!Kx_dev) return -5;
+    if (!Ky_dev) return -6;
+    if (!Kz_dev) return -7;
+    if (!V_dev) return -8;
+    if (!E0_dev) return -11;
+    if (!(T >= 0.0)) return -12;
+    if (Ec != Ec) return -13;
+    if (branch != 1 && branch != -1) return -14;
+    if (!(dt == dt)) return -15;
+    if (!Y_dev) return -16;
+    if (ldy < h->N) return -17;
+    if (!F_dev) return -18;
+    for (int k = 0; k < 5; ++k) if (!F_dev[k] || F_dev[k] == Y_dev || F_dev[k] == Yp_dev) return -18;
+    if (ldf < h->N) return -19;
+    if (!Yp_dev || Yp_dev == Y_dev) return -20;
+    if (ncols < 1 || ncols > h->N) return -21;
+    if (!n_dev) return -22;
+    if (!Delta_dev) return -23;
+    c128* F[5];
+    for (int k = 0; k < 5; ++k) F[k] = (c128*)F_dev[k];
+    NvtxRange r("eigh_tdslda_step");
+    return cuda_fail(h, launch_tdslda_step(h, (int)nx, (int)ny, (int)nz, Kx_dev, Ky_dev, Kz_dev, V_dev, g, mu, E0_dev, T, Ec, branch, dt,
+                                           (c128*)Y_dev, ldy, F, ldf, (c128*)Yp_dev, ncols, n_dev, (c128*)Delta_dev,
+                                           (cudaStream_t)stream), "tdslda_step");
+}
+
 int eigh_tridiagonalise_direct(eigh_handle_t h, void* A_dev, int64_t lda, double* d_dev, double* e_dev, void* stream) {
     int rc = ensure_ready(h);
     if (rc) return rc;
@@ -578,13 +642,14 @@ int eigh_solve_host(eigh_handle_t h, const void* A_host, int64_t lda, double* W_
     rc = stage_init(h);
     if (rc) return rc;
     cudaStream_t s = (cudaStream_t)stream;
+    const size_t es = h->real_dtype ? sizeof(double) : sizeof(c128);     // element size of A and Z
     NvtxRange whole("eigh_solve_host");
     // the copies run on the handle's copy stream, ordered against the caller's stream by events
     cudaError_t ce = cudaEventRecord(h->ev[0], s);
     if (ce == cudaSuccess) ce = cudaStreamWaitEvent(h->copy_stream, h->ev[0], 0);
     if (ce == cudaSuccess) {
         NvtxRange r("H2D A");
-        ce = stream_h2d(h, A_scratch_dev, A_host, (size_t)lda * h->N * sizeof(c128), h->copy_stream);
+        ce = stream_h2d(h, A_scratch_dev, A_host, (size_t)lda * h->N * es, h->copy_stream);
     }
     if (ce == cudaSuccess) ce = cudaEventRecord(h->ev[1], h->copy_stream);
     if (ce == cudaSuccess) ce = cudaStreamWaitEvent(s, h->ev[1], 0);
@@ -595,7 +660,7 @@ int eigh_solve_host(eigh_handle_t h, const void* A_host, int64_t lda, double* W_
         NvtxRange r("D2H W, Z");
         ce = stream_d2h(h, W_host, W_scratch_dev, (size_t)h->N * sizeof(double), h->copy_stream);
         if (ce == cudaSuccess)
-            ce = stream_d2h(h, Z_host, Z_scratch_dev, (size_t)h->N * h->nev * sizeof(c128), h->copy_stream);
+            ce = stream_d2h(h, Z_host, Z_scratch_dev, (size_t)h->N * h->nev * es, h->copy_stream);
     }
     if (ce == cudaSuccess) ce = cudaStreamSynchronize(h->copy_stream);
     if (ce != cudaSuccess) return set_err(h, 1000 + (int)ce, "eigh_solve_host D2H: %s", cudaGetErrorString(ce));

@@ -112,6 +112,14 @@ int phase_backtransform_band(eigh_handle_s* h, const double* Q, int64_t ldq, c12
                              cudaStream_t s);
 int phase_backtransform_full(eigh_handle_s* h, const c128* A, int64_t lda, c128* Z, int64_t ldz,
                              cudaStream_t s);
+// one TDSLDA step (tdslda.cu)
+int launch_tdslda_rhs(eigh_handle_s* h, int nx, int ny, int nz, const double* Kx, const double* Ky, const double* Kz,
+                      const double* V, const c128* Delta, double mu, const c128* Phi, int64_t ldp, int64_t ncols, c128* F,
+                      int64_t ldf, cudaStream_t s);
+int launch_tdslda_step(eigh_handle_s* h, int nx, int ny, int nz, const double* Kx, const double* Ky, const double* Kz,
+                       const double* V, double g, double mu, const double* E0, double T, double Ec, int branch, double dt,
+                       c128* Y, int64_t ldy, c128* const F[5], int64_t ldf, c128* Yp, int64_t ncols, double* n_out,
+                       c128* Delta, cudaStream_t s);
 // 1-stage variant (tridiag_direct.cu); A / Z are c128 or double according to h->real_dtype
 int phase_tridiagonalise_direct(eigh_handle_s* h, void* A, int64_t lda, double* d, double* e, cudaStream_t s);
 int phase_backtransform_direct(eigh_handle_s* h, const void* A, int64_t lda, const double* Q, int64_t ldq, void* Z,
