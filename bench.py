@@ -440,8 +440,37 @@ def main():
                                     "ms": ams, "algorithmic_bytes": 16.0 * N * N, "bound": "hbm",
                                     "achieved_gbs": 16.0 * N * N / ams / 1e6 if ams else None, "peak_gbs": hbm,
                                     "frac": (16.0 * N * N / ams / 1e6) / hbm if hbm and ams else None, "launches": 1}
+            # second workload: one TDSLDA step (eigh_tdslda_step) for a block of the states just computed.
+            # Algorithmic bytes per step and state: 2 evaluations x 8 x 16 N (three kinetic passes) + 2 combines x 7 x 16 N
+            # + 2 density passes x 16 N = 512 N bytes; HBM-bound.
+            nst = min(nev, 2048)
+            Kd = [torch.from_numpy(wl_mod.kinetic_1d(L)).to(dev) for L in pb.shape]
+            Vd = torch.from_numpy(pb.V).to(dev)
+            Yt = Zt[:nst].clone()
+            E0 = E[:nst].contiguous()
+            Dl0 = torch.from_numpy(np.ascontiguousarray(pb.Delta)).to(dev)
+            Fl = [solver.tdslda_rhs(pb.shape, Kd[0], Kd[1], Kd[2], Vd, Dl0, pb.mu, Yt) for _ in range(5)]
+            Ypt = torch.empty_like(Yt)
+            n_t = torch.empty(N // 2, dtype=torch.float64, device=dev)
+            D_t = torch.empty(N // 2, dtype=torch.complex128, device=dev)
+            ts = []
+            for it in range(4):
+                ev0.record(stream)
+                Fl = solver.tdslda_step(pb.shape, Kd[0], Kd[1], Kd[2], Vd, -1.0, pb.mu, E0, 1e-3, Yt, Fl, Ypt, n_t, D_t,
+                                        branch=branch)
+                ev1.record(stream)
+                torch.cuda.synchronize()
+                ts.append(ev0.elapsed_time(ev1))
+            sms = sorted(ts[1:])[len(ts[1:]) // 2]
+            sbytes = 512.0 * N * nst
+            epilogue["tdslda_step"] = {"op": "eigh_tdslda_step (Eq. 5, Eq. 8, ABM PECE step; %d states)" % nst, "ms": sms,
+                                       "launches": 20, "algorithmic_bytes": sbytes, "bound": "hbm",
+                                       "achieved_gbs": sbytes / sms / 1e6 if sms else None, "peak_gbs": hbm,
+                                       "frac": (sbytes / sms / 1e6) / hbm if hbm and sms else None,
+                                       "norm_drift": float((Yt.abs() ** 2).sum(dim=1).sub(1.0).abs().max().item())}
+            del Yt, Fl, Ypt
         except Exception as ex:   # reported, never hidden
-            epilogue = {"error": str(ex)[:200]}
+            epilogue = dict(epilogue or {}, error=str(ex)[:200])
 
     # ---- e2e: host buffers through eigh_solve_host.  A_host is PAGEABLE host memory of the full matrix; it is streamed
     # H2D through the handle's bounded pinned ring (2 x 256 MiB), W and Z come back the same way; all of it inside the
