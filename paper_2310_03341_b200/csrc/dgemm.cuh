@@ -93,6 +93,17 @@ static __global__ void __launch_bounds__(DG_NT, 2) dgemm_kernel(const DgemmArgs 
         vB[it] = gn < d.N;
         pB[it] = B + 2 * kp + (int64_t)(gn < d.N ? gn : 0) * p.ldb;
     }
+    // gathered columns of A: the indices of the NEXT requested k-block are fetched one request ahead, so that no
+    // cp.async address waits for an index load (the blocks are requested strictly in order 0, 1, 2, ...)
+    int cpre[NA];
+    auto fetch_idx = [&](int kb) {
+#pragma unroll
+        for (int it = 0; it < NA; ++it) {
+            const int k = kb * DG_BK + kA[it];
+            cpre[it] = (cidx && k < d.K) ? __ldg(cidx + k) : k;
+        }
+    };
+    fetch_idx(0);
     auto load_stage = [&](int stage, int kb) {
         double* As = smem + (size_t)stage * DG_STAGE;
         double* Bs = As + DG_BK * DG_SA;
@@ -103,8 +114,7 @@ static __global__ void __launch_bounds__(DG_NT, 2) dgemm_kernel(const DgemmArgs 
             int bytes = 0;
             const double* src = A;
             if (kA[it] < krem && bA[it]) {
-                const int64_t col = cidx ? (int64_t)__ldg(cidx + k0 + kA[it]) : (int64_t)(k0 + kA[it]);
-                src = pA[it] + col * p.lda;
+                src = pA[it] + (int64_t)cpre[it] * p.lda;
                 bytes = bA[it];
             }
             cp_async16(As + sA[it], src, bytes);
@@ -119,6 +129,7 @@ static __global__ void __launch_bounds__(DG_NT, 2) dgemm_kernel(const DgemmArgs 
             }
             cp_async16(Bs + sB[it], src, bytes);
         }
+        if (kb + 1 < nkb) fetch_idx(kb + 1);
     };
 
 #pragma unroll
