@@ -592,6 +592,9 @@ def main():
         "algorithmic_flops_per_launch": cw["p4a_flops"], "kernel_ms": sweep_ms, "launches_per_step": 1,
         "kernel_share_of_step": sweep_ms / ms_per_step if ms_per_step else None,
         "dominant_phase": PHASES[dominant],
+        "dominant_kernel_rule": "largest device time of a single kernel family per step: bt_sweep_kernel = all of p4a in one "
+                                "launch; the GEMM families of p1 / p4b (HEMM-lower, HER2K-lower, NN, CN instances of zgemm_kernel) "
+                                "stay at 12-17 % each (profiles/r02_launches_c4.md)",
         "peak_source": "FP64 tensor (DMMA) 148 SM x 64 FMA/clk x 2 x 1.965 GHz = 37.2 TFLOP/s, equal to the burst DMMA rate "
                        "measured on this pool (profiles/r01_fp64_peaks.md; cuBLAS ZGEMM 36.8); MEASURED_PEAKS.json has "
                        "no FP64 entry.  `frac` divides CREDITED flops (8 per complex multiply-add) by it; `frac_executed` "

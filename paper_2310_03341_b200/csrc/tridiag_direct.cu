@@ -292,28 +292,19 @@ __global__ void __launch_bounds__(HT_NT, 1) hetrd_panel_kernel(const HtArgs<T> a
                 cp_async_commit();
             };
             for (int s = 0; s < HT_STG - 1; ++s) issue(s);
-            // the two 64-element pieces of v a job multiplies with (threads 0..63: v_J, 64..127: v_I) are fetched from L2
-            // ONE JOB AHEAD into a register and parked in shared memory after the products of the current job, so that
-            // their latency hides behind a tile's worth of arithmetic instead of preceding every tile
-            auto vec_fetch = [&](long long j) -> T {
-                if (j >= njobs || tid >= 2 * HT_B) return S::zero();
-                int I, J, kind, nr, nc;
-                const T* src; int64_t ld;
-                job_src(j, I, J, kind, src, ld, nr, nc);
-                const int which = tid >> 6;                           // 0: v_J, 1: v_I
-                const int blk = which ? I : J;
-                return (kind >= 2 && which == 0) ? S::zero() : vget(j0 + blk * HT_B + r);
-            };
-            if (tid < 2 * HT_B) sm.vec[0][tid >> 6][r] = vec_fetch(0);
             for (long long j = 0; j < njobs; ++j) {
                 int I, J, kind, nr, nc;
                 const T* src; int64_t ld;
                 job_src(j, I, J, kind, src, ld, nr, nc);
                 const int par = (int)(j & 1);
+                if (tid < 2 * HT_B) {
+                    const int which = tid >> 6;                       // 0: v_J, 1: v_I
+                    const int blk = which ? I : J;
+                    sm.vec[par][which][r] = (kind >= 2 && which == 0) ? S::zero() : vget(j0 + blk * HT_B + r);
+                }
                 cp_async_wait<HT_STG - 2>();
                 __syncthreads();
                 issue(j + HT_STG - 1);
-                const T vnext = vec_fetch(j + 1);                     // consumed after the products below
                 const T* St = sm.tile[j % HT_STG];
                 const T* vJ = sm.vec[par][0];
                 const T* vI = sm.vec[par][1];
@@ -338,7 +329,6 @@ __global__ void __launch_bounds__(HT_NT, 1) hetrd_panel_kernel(const HtArgs<T> a
                 }
                 sm.red[0][q][r] = accr;
                 sm.red[1][q][r] = accc;
-                if (tid < 2 * HT_B) sm.vec[par ^ 1][tid >> 6][r] = vnext;   // (that buffer was last read by job j - 1)
                 __syncthreads();
                 if (tid < 2 * HT_B) {
                     const int which = tid >> 6;
