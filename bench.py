@@ -247,6 +247,10 @@ def main():
     ap.add_argument("--method", type=int, default=2, choices=(1, 2),
                     help="2 = two-stage solver (the hot path, default); 1 = the 1-stage variant of SURVEY.md 8(f)2 "
                          "(PAPER.md:148 steps i-iii; use with --config 0..2)")
+    ap.add_argument("--shard", action="store_true",
+                    help="N > 1 only, NOT the default (the path is 'replicas only'): strong-scaling run of ONE problem with "
+                         "the back-transformations sharded by eigenvector columns (option col_begin; S1-S3 replicated, Z "
+                         "left distributed, no collective on the data path) -- SURVEY.md 8(f)3 first slice, DESIGN.md 3.10")
     ap.add_argument("--real", action="store_true",
                     help="real-symmetric FP64 path (needs --method 1 and a real matrix: --config 0)")
     args = ap.parse_args()
@@ -285,6 +289,13 @@ def main():
     for kv in args.opt:
         key, val = kv.split("=")
         opts[key] = int(val)
+    nev_total = nev
+    sharded = args.shard and world > 1
+    if sharded:
+        from paper_2310_03341_b200 import shard as shard_mod
+        c0, c1 = shard_mod.column_shards(nev_total, world)[rank]
+        nev = max(c1 - c0, 1)
+        opts["col_begin"] = min(c0, N - nev)
     solver = binding.Eigh(N, nev, device=dev, **opts)
     b = solver.band_width                                    # read from the handle (eigh_get_option)
     mat_bytes = N * N * 16
@@ -354,6 +365,8 @@ def main():
     clocks = sampler.stop(t0, t1) if rank == 0 else None
     ms_per_step = total_ms / args.steps
     value_s = replica_value_s(ms_per_step, world)        # seconds per eigensolve, whole job (replicas)
+    if sharded:
+        value_s = ms_per_step / 1e3                      # one problem solved by all ranks together
     dc_flops, dc_kept = solver.dc_stats()                # S3 merge statistics of the last solve
 
     # ---- quick validity check of the last solve (device side, independent ZGEMM by torch)
@@ -607,7 +620,9 @@ def main():
         "hbm_peak_gbs": hbm,
         "p2_hbm_frac_credited": (cw["p2_bytes"] / ph[1] / 1e6) / hbm if ph[1] and hbm else None,
     }
-    cfg = config_dict(w, nev, nev_rule, b)
+    cfg = config_dict(w, nev_total, nev_rule, b)
+    if sharded:
+        cfg["parallelism"] = "column-sharded back-transformations over %d ranks (rank 0: %d of %d columns)" % (world, nev, nev_total)
     if args.method == 1:
         # 1-stage variant.  Dominant kernel = hetrd_panel_kernel (one cooperative launch per 64-column
         # panel, all inside phase 0 together with the HER2K / SYR2K GEMMs): HBM-bound, algorithmic bytes = the lower
@@ -637,7 +652,8 @@ def main():
         cfg["dtype"] = "f64 real symmetric" if args.real else "c128"
     line = {
         "metric": "eigh_time_s", "value": value_s, "unit": "s", "n_gpus": world, "steps": args.steps,
-        "warmup": args.warmup, "ms_per_step": ms_per_step, "higher_is_better": False, "scaling": "weak",
+        "warmup": args.warmup, "ms_per_step": ms_per_step, "higher_is_better": False,
+        "scaling": "strong" if sharded else "weak",
         "vs_baseline": None, "dtype": "f64" if args.real else "c128", "data": "synthetic",
         "config": cfg,
         "clocks": clocks, "e2e": e2e, "gpu_launches": launches, "phases": phase_report, "roofline": roofline,

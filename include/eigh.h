@@ -52,6 +52,9 @@ int eigh_create(eigh_handle_t* h, int64_t N, int64_t nev);
  * co-resident block, the default), "bc_dual_steps" (S2: sweeps with at least this many chase steps run on the variant
  * with two thread blocks per SM and no publisher warp; 0 = never, the default -- it measured 2-8 % slower at N = 27648 /
  * 49152, the kernel being bound by L2 traffic rather than by occupancy), "band_width" (64: the only width S2 / S4a are built for; anything else is -3),
+ * "col_begin" (first eigenvector column returned: Z gets the eigenvectors of W[col_begin .. col_begin + nev) instead of
+ * W[0 .. nev); W still holds all N eigenvalues.  This is the column shard of the back-transformations, the first slice of
+ * a multi-GPU solve: S1-S3 are replicated, every rank back-transforms its own slab-aligned column range; default 0),
  * "method" (2 = the two-stage solver, the default; 1 = the ONE-STAGE solver of PAPER.md:148 steps i-iii: direct
  * blocked Householder tridiagonalisation, D&C, one back-transformation -- the solver the paper benchmarks in
  * Figs. 3-4), "dtype" (0 = complex Hermitian c128, the default; 1 = REAL SYMMETRIC FP64:

@@ -157,6 +157,9 @@ int eigh_set_option(eigh_handle_t h, const char* key, int64_t value) {
     } else if (!strcmp(key, "bc_dual_steps")) {
         if (value < 0 || value > (1 << 20)) return set_err(h, -3, "bc_dual_steps must be in [0, 2^20]");
         h->bc_dual_steps = (int)value;
+    } else if (!strcmp(key, "col_begin")) {
+        if (value < 0 || value + h->nev > h->N) return set_err(h, -3, "col_begin must satisfy 0 <= col_begin <= N - nev");
+        h->col0 = (int)value;
     } else if (!strcmp(key, "method")) {
         if (value != 1 && value != 2) return set_err(h, -3, "method must be 1 (one-stage) or 2 (two-stage)");
         if (value == 2 && h->real_dtype) return set_err(h, -3, "the real-symmetric path exists for method = 1 only");
@@ -194,6 +197,7 @@ int eigh_get_option(eigh_handle_t h, const char* key, int64_t* value) {
     else if (!strcmp(key, "hemm_waves")) *value = h->hemm_waves;
     else if (!strcmp(key, "bc_grid")) *value = h->bc_grid;
     else if (!strcmp(key, "bc_dual_steps")) *value = h->bc_dual_steps;
+    else if (!strcmp(key, "col_begin")) *value = h->col0;
     else if (!strcmp(key, "method")) *value = h->method;
     else if (!strcmp(key, "dtype")) *value = h->real_dtype;
     else if (!strcmp(key, "ht_grid")) *value = h->ht_grid;

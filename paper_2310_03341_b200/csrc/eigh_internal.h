@@ -50,6 +50,7 @@ struct eigh_handle_s {
     int bt_chain;   // S4a: consecutive passes of one slab scheduled back to back (0 = auto)
     int bc_grid;    // S2: CTAs of the bulge-chasing kernel (0 = all that are co-resident)
     int bc_dual_steps;  // S2: sweeps with at least this many chase steps run two thread blocks per SM (0 = never)
+    int col0;       // first eigenvector column this handle returns (column shard of the back-transformations; default 0)
     int method;     // 2 = two-stage (default), 1 = one-stage direct tridiagonalisation
     int real_dtype; // 0 = complex Hermitian (c128), 1 = real symmetric (double); real needs method = 1
     int ht_grid;    // 1-stage: thread blocks of the panel kernel (0 = all that are co-resident)

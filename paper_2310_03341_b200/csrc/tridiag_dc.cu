@@ -613,23 +613,24 @@ __global__ void __launch_bounds__(256) dc_finish_kernel(const MergeDesc* __restr
 }
 
 // final: W[rank] = d, Qout[:, rank] = Q[:, j] for rank < nev
-__global__ void __launch_bounds__(256) dc_output_kernel(int N, int nev, const int* __restrict__ perm, const double* __restrict__ dcur,
+__global__ void __launch_bounds__(256) dc_output_kernel(int N, int col0, int nev, const int* __restrict__ perm, const double* __restrict__ dcur,
                                                         const double* __restrict__ Q, int64_t ldq, double* __restrict__ W,
                                                         double* __restrict__ Qout, int64_t ldo,
                                                         const double* __restrict__ esgn) {
     const int rank = blockIdx.x;
     const int j = perm[rank];
     if (threadIdx.x == 0) W[rank] = dcur[j];
-    if (rank >= nev) return;
+    if (rank < col0 || rank >= col0 + nev) return;           // (col0 > 0: this handle's column shard)
     const double* a = Q + (int64_t)j * ldq;
-    double* b = Qout + (int64_t)rank * ldo;
+    double* b = Qout + (int64_t)(rank - col0) * ldo;
     for (int r = threadIdx.x; r < N; r += 256) b[r] = esgn[r] * a[r];
 }
 
 // ------------------------------------------------------------------ driver
 int phase_tridiag_dc(eigh_handle_s* h, const double* d, const double* e, double* W, double* Qout, int64_t ldo,
                      cudaStream_t st, int* nfail) {
-    const int N = (int)h->N, nev = (int)h->nev;
+    const int N = (int)h->N, nev = (int)h->nev, col0 = h->col0;
+    const int nwant = col0 + nev;                             // eigenvectors 0 .. nwant-1 must exist after the last merge
     DcBufs B = dc_carve(ws_ptr<char>(h, h->plan.dc), N);
     const int64_t ldq = B.ldq;
     // ---- tree (host): L = 2^p leaves, even boundaries
@@ -701,9 +702,9 @@ int phase_tridiag_dc(eigh_handle_s* h, const double* d, const double* e, double*
         dc_zhat_kernel<<<dim3(gx128, cnt), 128, 0, st>>>(dd, B.kcount, B.dk, B.zk, B.org, B.mu, B.zhat);
         dc_build_u_kernel<<<dim3(maxn, cnt), 256, 0, st>>>(dd, B.kcount, B.dk, B.org, B.mu, B.zhat, B.upos, B.U, ldq);
         const int* kn = nullptr;
-        if (nev < N && lv + 1 == level_cnt.size() && cnt == 1) {
+        if (nwant < N && lv + 1 == level_cnt.size() && cnt == 1) {
             EIGH_CUDA_OK(cudaMemsetAsync(B.fail + 16, 0, sizeof(int), st));
-            dc_wanted_kernel<<<gx256, 256, 0, st>>>(dd, B.kcount, B.df_idx, dcur, B.lam, nev, B.fail + 16);
+            dc_wanted_kernel<<<gx256, 256, 0, st>>>(dd, B.kcount, B.df_idx, dcur, B.lam, nwant, B.fail + 16);
             ++h->launches;
             kn = B.fail + 16;          // second counter in the 256-byte block of `fail`
         }
@@ -723,7 +724,7 @@ int phase_tridiag_dc(eigh_handle_s* h, const double* d, const double* e, double*
     }
     // ---- final ascending order
     dc_rank_kernel<<<dim3((unsigned)ceil_div(N, 256), 1), 256, 0, st>>>(B.desc + final_desc, dcur, B.perm);
-    dc_output_kernel<<<N, 256, 0, st>>>(N, nev, B.perm, dcur, Qcur, ldq, W, Qout, ldo, B.esgn);
+    dc_output_kernel<<<N, 256, 0, st>>>(N, col0, nev, B.perm, dcur, Qcur, ldq, W, Qout, ldo, B.esgn);
     h->launches += 2;
     int fail = 0;
     double stats[32 * 3];
