@@ -44,6 +44,7 @@
 namespace eigh {
 
 constexpr bool BT_QPLANE = true;    // stage tiles carry q = vx - vy (a third bulk copy, 16 KB): no V-side adds in the two 3-product forms
+constexpr bool BT_Y1_SPLIT = false;  // Y1 = V^H Z: one accumulator chain per 3M sum (false) or one per k-step parity (true: 6 more adds per block)
 constexpr int BT_RING8 = 3;         // stages of the ring for GS = 8 (with the q plane there is room for three)
 constexpr int BT_B = 64;            // band width (reflector length)
 constexpr int BT_P = 32;            // sweeps per pass
@@ -293,9 +294,9 @@ __device__ __forceinline__ void bt_apply_step(const c128* __restrict__ Vs, const
                             if constexpr (bt_qplane(GS)) qv = Qs[(8 * p + 2 * t + h) + (8 * cb + g) * BT_LDV];
                         }
                         if constexpr (!bt_qplane(GS)) qv = v.x - v.y;
-                        dmma_p(s1[c][h], ar, v.x);
-                        dmma_p(s2[c][h], ai, v.y);
-                        dmma_p(s3[c][h], as, qv);
+                        dmma_p(s1[c][BT_Y1_SPLIT ? h : 0], ar, v.x);
+                        dmma_p(s2[c][BT_Y1_SPLIT ? h : 0], ai, v.y);
+                        dmma_p(s3[c][BT_Y1_SPLIT ? h : 0], as, qv);
                     }
                 }
             }
@@ -305,7 +306,9 @@ __device__ __forceinline__ void bt_apply_step(const c128* __restrict__ Vs, const
         for (int c = 0; c < NB; ++c)
 #pragma unroll
             for (int e = 0; e < 2; ++e) {
-                const double t1 = s1[c][0][e] + s1[c][1][e], t2 = s2[c][0][e] + s2[c][1][e], t3 = s3[c][0][e] + s3[c][1][e];
+                const double t1 = BT_Y1_SPLIT ? s1[c][0][e] + s1[c][1][e] : s1[c][0][e];
+                const double t2 = BT_Y1_SPLIT ? s2[c][0][e] + s2[c][1][e] : s2[c][0][e];
+                const double t3 = BT_Y1_SPLIT ? s3[c][0][e] + s3[c][1][e] : s3[c][0][e];
                 ar1[c][e] = t1 + t2;
                 ai1[c][e] = (t3 - t1) + t2;
             }
@@ -497,6 +500,7 @@ __global__ void __launch_bounds__(BT_NT, 1) bt_sweep_kernel(const BtSweepArgs a)
 #pragma unroll
     for (int p = 0; p < BT_NBLK; ++p) zr[p][0] = zr[p][1] = zi[p][0] = zi[p][1] = 0.0;
     uint32_t zphase = 0;
+    int pred_seen = 0;                  // progress of the predecessor unit as last observed by this warp
 
     for (uint32_t it = 0;; ++it) {
         const int slot = it % BT_STAGES;
@@ -517,9 +521,11 @@ __global__ void __launch_bounds__(BT_NT, 1) bt_sweep_kernel(const BtSweepArgs a)
         if (hh.flags & 1) {
             // first step of the unit: the whole 96-row window straight from global memory.  Its last rows are
             // finalised by step 0 of the predecessor.
+            pred_seen = 0;
             if (hh.nk_pred > 0) {
-                if (lane == 0) while (bt_ld_acquire(predprog) < 1) {}
-                __syncwarp();
+                int v = 0;
+                if (lane == 0) do { v = bt_ld_acquire(predprog); } while (v < 1);
+                pred_seen = __shfl_sync(0xffffffffu, v, 0);
                 asm volatile("fence.proxy.async.global;" ::: "memory");  // rows were written through the async proxy
             }
 #pragma unroll
@@ -543,8 +549,14 @@ __global__ void __launch_bounds__(BT_NT, 1) bt_sweep_kernel(const BtSweepArgs a)
         const int nin = last ? 0 : min(BT_B, nrows - BT_WR);          // incoming rows (may be <= 0 near the end)
         if (nin > 0) {
             if (hh.nk_pred > 0) {
+                // the predecessor publishes every eighth step: one acquire usually covers the next steps too, so the
+                // counter is only read again when the value seen last is not enough
                 const int need = min(hh.k + 2, hh.nk_pred);
-                if (lane == 0) while (bt_ld_acquire(predprog) < need) {}
+                if (pred_seen < need) {
+                    int v = 0;
+                    if (lane == 0) do { v = bt_ld_acquire(predprog); } while (v < need);
+                    pred_seen = __shfl_sync(0xffffffffu, v, 0);
+                }
             }
             if (lane < 8) bulk_wait_read<0>();                         // the tile's previous bulk stores have read it
             if (lane == 0) {
@@ -609,13 +621,14 @@ __global__ void __launch_bounds__(BT_NT, 1) bt_sweep_kernel(const BtSweepArgs a)
             asm volatile("fence.proxy.async.shared::cta;" ::: "memory");     // the tile was written by generic stores
             __syncwarp();
             if (issuer) bulk_s2g(a.Z + (int64_t)mycol * a.ldz + R0, Zs + lane * BT_LDZ, BT_B * (uint32_t)sizeof(c128));
+            const bool publish = hh.k > 0 && (hh.k & 15) == 0;      // every 16th step: the release fence is not free
             if (lane < 8) {
                 bulk_commit();
-                bulk_wait<1>();                                     // the stores of step k-1 are complete
+                if (publish) bulk_wait<1>();                        // the stores of the steps before this one are complete
             }
             __syncwarp();
             // ---- publish the previous step
-            if (hh.k > 0 && (hh.k & 1) == 0) {                      // every second step: the release fence is not free
+            if (publish) {
                 if (lane == 0) bt_st_release(myprog, hh.k);
                 __syncwarp();
             }
