@@ -316,18 +316,28 @@ __device__ __forceinline__ void bt_apply_step(const c128* __restrict__ Vs, const
         double yr[NB][2], yi[NB][2];
 #pragma unroll
         for (int co = 0; co < NB; ++co) {
-            yr[co][0] = yr[co][1] = yi[co][0] = yi[co][1] = 0.0;
+            // two accumulator pairs (one per k-step parity h): the dependent chain Y1 -> Y -> Z is two DMMAs deep instead of four
+            double yra[2] = {0.0, 0.0}, yia[2] = {0.0, 0.0}, yrb[2] = {0.0, 0.0}, yib[2] = {0.0, 0.0};
 #pragma unroll
             for (int ci = co; ci < NB; ++ci)
 #pragma unroll
                 for (int h = 0; h < 2; ++h) {
                     const c128 tt = Ts[s * GS * (GS + 1) + (8 * co + g) + (8 * ci + 2 * t + h) * (GS + 1)];
                     const double ar = ar1[ci][h], ai = ai1[ci][h], nai = -ai;
-                    dmma_p(yr[co], ar, tt.x);
-                    dmma_p(yi[co], ai, tt.x);
-                    dmma_p(yr[co], nai, tt.y);
-                    dmma_p(yi[co], ar, tt.y);
+                    if (h == 0) {
+                        dmma_p(yra, ar, tt.x);
+                        dmma_p(yia, ai, tt.x);
+                        dmma_p(yra, nai, tt.y);
+                        dmma_p(yia, ar, tt.y);
+                    } else {
+                        dmma_p(yrb, ar, tt.x);
+                        dmma_p(yib, ai, tt.x);
+                        dmma_p(yrb, nai, tt.y);
+                        dmma_p(yib, ar, tt.y);
+                    }
                 }
+            yr[co][0] = yra[0] + yrb[0]; yr[co][1] = yra[1] + yrb[1];
+            yi[co][0] = yia[0] + yib[0]; yi[co][1] = yia[1] + yib[1];
         }
         // ---- Z += Y V   (m = column of Z, n = row, k = reflector)
         if constexpr (bt_qplane(GS)) {
