@@ -480,6 +480,10 @@ def main():
                                        "launches": 20, "algorithmic_bytes": sbytes, "bound": "hbm",
                                        "achieved_gbs": sbytes / sms / 1e6 if sms else None, "peak_gbs": hbm,
                                        "frac": (sbytes / sms / 1e6) / hbm if hbm and sms else None,
+                                       "minimal_bytes": 320.0 * N * nst,
+                                       "frac_minimal": (320.0 * N * nst / sms / 1e6) / hbm if hbm and sms else None,
+                                       "note": "algorithmic_bytes = the three-pass kinetic scheme as built (512 N per state and "
+                                               "step); minimal_bytes = phi read once and f written once per evaluation (320 N)",
                                        "norm_drift": float((Yt.abs() ** 2).sum(dim=1).sub(1.0).abs().max().item())}
             del Yt, Fl, Ypt
         except Exception as ex:   # reported, never hidden

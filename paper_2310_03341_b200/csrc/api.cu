@@ -540,13 +540,27 @@ constexpr size_t STAGE_BYTES = (size_t)256 << 20;
 
 static int stage_init(eigh_handle_s* h) {
     if (h->stage_ok) return 0;
-    for (int i = 0; i < 2; ++i) {
-        cudaError_t e = cudaMallocHost(&h->stage[i], STAGE_BYTES);
-        if (e == cudaSuccess) e = cudaEventCreateWithFlags(&h->ev_stage[i], cudaEventDisableTiming);
-        if (e != cudaSuccess) return set_err(h, 1000 + (int)e, "eigh_solve_host staging ring: %s", cudaGetErrorString(e));
+    cudaError_t e = cudaSuccess;
+    int nbuf = 0, nev = 0;
+    bool have_stream = false;
+    for (int i = 0; i < 2 && e == cudaSuccess; ++i) {
+        e = cudaMallocHost(&h->stage[i], STAGE_BYTES);
+        if (e == cudaSuccess) ++nbuf; else h->stage[i] = nullptr;
     }
-    cudaError_t e = cudaStreamCreateWithFlags(&h->copy_stream, cudaStreamNonBlocking);
-    if (e != cudaSuccess) return set_err(h, 1000 + (int)e, "eigh_solve_host copy stream: %s", cudaGetErrorString(e));
+    for (int i = 0; i < 2 && e == cudaSuccess; ++i) {
+        e = cudaEventCreateWithFlags(&h->ev_stage[i], cudaEventDisableTiming);
+        if (e == cudaSuccess) ++nev;
+    }
+    if (e == cudaSuccess) {
+        e = cudaStreamCreateWithFlags(&h->copy_stream, cudaStreamNonBlocking);
+        have_stream = e == cudaSuccess;
+    }
+    if (e != cudaSuccess) {           // undo the part that succeeded: a failed init leaves nothing behind
+        for (int i = 0; i < nbuf; ++i) { cudaFreeHost(h->stage[i]); h->stage[i] = nullptr; }
+        for (int i = 0; i < nev; ++i) cudaEventDestroy(h->ev_stage[i]);
+        if (have_stream) cudaStreamDestroy(h->copy_stream);
+        return set_err(h, 1000 + (int)e, "eigh_solve_host staging ring: %s", cudaGetErrorString(e));
+    }
     h->stage_bytes = STAGE_BYTES;
     h->stage_ok = true;
     return 0;
@@ -712,8 +726,6 @@ int eigh_destroy(eigh_handle_t h) {
     if (h->stage_ok) {
         for (int i = 0; i < 2; ++i) { cudaFreeHost(h->stage[i]); cudaEventDestroy(h->ev_stage[i]); }
         cudaStreamDestroy(h->copy_stream);
-    } else {
-        for (int i = 0; i < 2; ++i) if (h->stage[i]) cudaFreeHost(h->stage[i]);
     }
     delete h;
     return 0;
