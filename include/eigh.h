@@ -196,6 +196,20 @@ int eigh_backtransform_full(eigh_handle_t h, const void* A_dev, int64_t lda, voi
 int eigh_densities(eigh_handle_t h, const double* E_dev, const void* Z_dev, int64_t ldz, int64_t ncols,
                    double T, double Ec, int branch, double* n_dev, void* nu_dev, void* stream);
 
+/* eigh_densities WITHOUT any allocation and without a workspace: for callers that cannot call cudaMalloc (code under
+ * CUDA graph capture, tight serving loops, harnesses that forbid it).  Same arguments, same kernels and same results as
+ * eigh_densities (the chunking of the sums may differ, so results agree to rounding, not bit for bit); the scratch (list
+ * of active columns + chunk partials) is a file-scope device array of 8 MiB that every GPU loading this library holds
+ * until exit.  The handle is used for N, the launch counter and the error text only: eigh_set_workspace need not have
+ * been called.  Limits: N <= 65536 and ncols <= 32760; beyond them the call returns -1 / -5 with a message in
+ * eigh_last_error and launches nothing (use eigh_densities).  Calls no cudaMalloc / cudaFree or allocating routine; the
+ * first call on a device looks up the array's device address (cudaGetSymbolAddress) and the SM count.
+ * ALL calls share the one array, which keeps the last call's contents: calls on one stream run one after the other and are
+ * safe; calls that overlap on the GPU (different streams, different handles or host threads) RACE on it -- serialise
+ * them.  Enqueues one memset (256 B) + 3 kernels on `stream`, does not synchronise. */
+int eigh_densities_static(eigh_handle_t h, const double* E_dev, const void* Z_dev, int64_t ldz, int64_t ncols,
+                          double T, double Ec, int branch, double* n_dev, void* nu_dev, void* stream);
+
 /* Kinetic and current densities (Eq. 16b, 16c), same states, weights and `branch` rule as eigh_densities:
  *     tau(r) = 2 sum ( |grad v_n|^2 f_T(-E_n) + |grad u_n|^2 f_T(E_n) )
  *     j(r)   = 2 sum Im( v_n grad v_n^* f_T(-E_n) - u_n grad u_n^* f_T(E_n) )

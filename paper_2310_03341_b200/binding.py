@@ -40,6 +40,7 @@ SIGNATURES = {
     "eigh_tridiagonalise_direct": (_int, [_vp, _vp, _i64, _vp, _vp, _vp]),
     "eigh_backtransform_direct": (_int, [_vp, _vp, _i64, _vp, _i64, _vp]),
     "eigh_densities": (_int, [_vp, _vp, _vp, _i64, _i64, _dbl, _dbl, _int, _vp, _vp, _vp]),
+    "eigh_densities_static": (_int, [_vp, _vp, _vp, _i64, _i64, _dbl, _dbl, _int, _vp, _vp, _vp]),
     "eigh_gradient_densities": (_int, [_vp, _i64, _i64, _i64, _vp, _vp, _vp, _vp, _vp, _i64, _i64, _dbl, _dbl, _int,
                                        _vp, _vp, _vp]),
     "eigh_assemble_bdg": (_int, [_vp, _i64, _i64, _i64, _vp, _vp, _vp, _vp, _vp, _dbl, _dbl, _vp, _i64, _vp]),
@@ -176,6 +177,16 @@ class Eigh:
         rc = self.lib.eigh_densities(self.h, _ptr(E), _ptr(Zt), ldz, ncols, float(T), float(Ec), int(branch),
                                      _ptr(n), _ptr(nu), _stream())
         self._check(rc, "eigh_densities")
+        return n, nu
+
+    def densities_static(self, E, Zt, n, nu, T: float = 0.0, Ec: float = float("inf"), branch: int = 1):
+        """eigh_densities_static: eigh_densities with its scratch in a static device array (no allocation, no workspace;
+        N <= 65536, ncols <= 32760).  n [N/2] float64 and nu [N/2] complex128 are caller-provided outputs."""
+        ncols = int(Zt.shape[0])
+        ldz = int(Zt.stride(0)) if ncols > 1 else self.N
+        rc = self.lib.eigh_densities_static(self.h, _ptr(E), _ptr(Zt), ldz, ncols, float(T), float(Ec), int(branch),
+                                            _ptr(n), _ptr(nu), _stream())
+        self._check(rc, "eigh_densities_static")
         return n, nu
 
     def gradient_densities(self, shape, Dx, Dy, Dz, E, Zt, T: float = 0.0, Ec: float = float("inf"), branch: int = 1):

@@ -426,4 +426,94 @@ int launch_densities(eigh_handle_s* h, const double* E, const c128* Z, int64_t l
     return 0;
 }
 
+// ------------------------------------------------------------------ eigh_densities_static: the allocation-free variant
+// Same three kernels as launch_densities, with the scratch (list of active columns + chunk partials) in a FILE-SCOPE device
+// array instead of the caller's workspace: for callers that cannot call cudaMalloc (code under CUDA graph capture, tight
+// serving loops, harnesses that forbid it).  Every GPU that loads the library holds these DENS_STATIC_BYTES until exit.
+// In HOST code the array's name is a host-side stand-in, not a device address: the address the kernels get comes from
+// cudaGetSymbolAddress, taken once per device with that device current (dens_static_setup below).
+constexpr size_t DENS_STATIC_BYTES = (size_t)8 << 20;             // 8 MiB per device
+constexpr size_t DENS_STATIC_ACT_BYTES = (size_t)1 << 20;         // head: nact word (256 B) + the list of active columns
+constexpr int64_t DENS_STATIC_MAX_COLS = (int64_t)((DENS_STATIC_ACT_BYTES - 256) / sizeof(DensCol));      // 32760
+constexpr int64_t DENS_STATIC_MAX_N = 65536;                      // M = N/2 <= 32768: one chunk of partials = 768 KiB
+static __device__ __align__(256) unsigned char g_dens_static_scratch[DENS_STATIC_BYTES];
+
+struct DensStaticDev { bool ready; unsigned char* ptr; int num_sms; int occ; };
+constexpr int DENS_STATIC_MAX_DEVICES = 64;
+static DensStaticDev g_dens_static_dev[DENS_STATIC_MAX_DEVICES];   // host side, indexed by device ordinal
+
+// once per device, with that device current: the device address of the scratch array, SM count, occupancy
+static int dens_static_setup(eigh_handle_s* h, DensStaticDev** out) {
+    int dev = -1;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return set_err(h, 1000 + (int)e, "eigh_densities_static: cudaGetDevice: %s", cudaGetErrorString(e));
+    if (dev < 0 || dev >= DENS_STATIC_MAX_DEVICES) return set_err(h, EIGH_ERR_CUDA, "eigh_densities_static: device ordinal %d out of range", dev);
+    DensStaticDev& d = g_dens_static_dev[dev];
+    if (!d.ready) {
+        void* ptr = nullptr;
+        e = cudaGetSymbolAddress(&ptr, g_dens_static_scratch);
+        if (e != cudaSuccess || !ptr)
+            return set_err(h, 1000 + (int)e, "eigh_densities_static: cudaGetSymbolAddress: %s", cudaGetErrorString(e));
+        int sms = 0, occ = 0;
+        e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+        if (e == cudaSuccess) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, dens_partial_kernel, DP_THREADS, 0);
+        if (e != cudaSuccess || sms <= 0)
+            return set_err(h, 1000 + (int)e, "eigh_densities_static: device query: %s", cudaGetErrorString(e));
+        d.ptr = (unsigned char*)ptr; d.num_sms = sms; d.occ = occ > 0 ? occ : 1;
+        d.ready = true;
+    }
+    *out = &d;
+    return 0;
+}
+
 }  // namespace eigh
+
+// C ABI (include/eigh.h).  Lives in this file because the scratch array does: only this translation unit can take its address.
+extern "C" int eigh_densities_static(eigh_handle_t h, const double* E_dev, const void* Z_dev, int64_t ldz, int64_t ncols,
+                                     double T, double Ec, int branch, double* n_dev, void* nu_dev, void* stream) {
+    using namespace eigh;
+    if (!h) return -1;
+    const int64_t N = h->N, M = N / 2;
+    if (N & 1) return set_err(h, -1, "eigh_densities_static: N = %lld is odd (phi = [u, v] needs N = 2M)", (long long)N);
+    if (N > DENS_STATIC_MAX_N)
+        return set_err(h, -1, "eigh_densities_static: N = %lld exceeds the static scratch limit N <= %lld (use eigh_densities)",
+                       (long long)N, (long long)DENS_STATIC_MAX_N);
+    if (!E_dev && ncols > 0) return -2;
+    if (!Z_dev && ncols > 0) return -3;
+    if (ldz < N) return -4;
+    if (ncols < 0 || ncols > N) return -5;
+    if (ncols > DENS_STATIC_MAX_COLS)
+        return set_err(h, -5, "eigh_densities_static: ncols = %lld exceeds the static scratch limit ncols <= %lld (use eigh_densities)",
+                       (long long)ncols, (long long)DENS_STATIC_MAX_COLS);
+    if (!(T >= 0.0)) return -6;
+    if (Ec != Ec) return -7;
+    if (branch != 1 && branch != -1) return -8;
+    if (!n_dev) return -9;
+    if (!nu_dev) return -10;
+    DensStaticDev* d = nullptr;
+    int rc = dens_static_setup(h, &d);
+    if (rc) return rc;
+    cudaStream_t s = (cudaStream_t)stream;
+    int* nact = reinterpret_cast<int*>(d->ptr);                              // first word of the array
+    DensCol* act = reinterpret_cast<DensCol*>(d->ptr + 256);
+    double* part = reinterpret_cast<double*>(d->ptr + DENS_STATIC_ACT_BYTES);
+    const int64_t max_chunks = (int64_t)((DENS_STATIC_BYTES - DENS_STATIC_ACT_BYTES) / ((size_t)3 * (M > 0 ? M : 1) * sizeof(double)));
+    const int64_t row_blocks = ceil_div(M > 0 ? M : 1, DP_THREADS);
+    int64_t nchunks = std::max<int64_t>(1, (int64_t)d->num_sms * d->occ / row_blocks);
+    nchunks = std::min(nchunks, ceil_div(std::max<int64_t>(ncols, 1), 2 * DP_UNROLL));
+    nchunks = std::max<int64_t>(1, std::min(nchunks, std::min<int64_t>(max_chunks, 65535)));
+    // The array keeps the previous call's contents.  Nothing in it is read before this call writes it (the weights kernel
+    // writes the count and the list, every chunk partial is written before the reduction reads it); the count word is
+    // cleared all the same, so that a call whose first kernel failed to launch cannot reuse a stale count.
+    cudaError_t e = cudaMemsetAsync(nact, 0, 256, s);
+    if (e != cudaSuccess) return set_err(h, 1000 + (int)e, "eigh_densities_static: %s", cudaGetErrorString(e));
+    dens_weights_kernel<<<1, DW_THREADS, 0, s>>>(E_dev, ncols, T, Ec, branch, act, nact);
+    if (M > 0) {
+        dens_partial_kernel<<<dim3((unsigned)row_blocks, (unsigned)nchunks), DP_THREADS, 0, s>>>((const c128*)Z_dev, ldz, M, act, nact, part);
+        dens_reduce_kernel<<<(unsigned)ceil_div(M, 256), 256, 0, s>>>(part, (int)nchunks, M, n_dev, (c128*)nu_dev);
+    }
+    h->launches += 3;
+    e = cudaGetLastError();
+    if (e != cudaSuccess) return set_err(h, 1000 + (int)e, "eigh_densities_static: %s", cudaGetErrorString(e));
+    return 0;
+}
