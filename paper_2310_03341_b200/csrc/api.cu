@@ -113,6 +113,7 @@ int eigh_create(eigh_handle_t* out, int64_t N, int64_t nev) {
     h->panel_smem = 1;
     h->panel_rows_min = 96;
     h->hemm_waves = 14;
+    h->bc_variant = 3;
     h->method = 2;
     h->real_dtype = 0;
     h->num_sms = 0;
@@ -154,6 +155,9 @@ int eigh_set_option(eigh_handle_t h, const char* key, int64_t value) {
     } else if (!strcmp(key, "bc_grid")) {
         if (value < 0 || value > 4096) return set_err(h, -3, "bc_grid must be in [0, 4096]");
         h->bc_grid = (int)value;
+    } else if (!strcmp(key, "bc_variant")) {
+        if (value != 0 && value != 2 && value != 3) return set_err(h, -3, "bc_variant must be 0, 2 or 3");
+        h->bc_variant = (int)value;
     } else if (!strcmp(key, "bc_dual_steps")) {
         if (value < 0 || value > (1 << 20)) return set_err(h, -3, "bc_dual_steps must be in [0, 2^20]");
         h->bc_dual_steps = (int)value;
@@ -196,6 +200,7 @@ int eigh_get_option(eigh_handle_t h, const char* key, int64_t* value) {
     else if (!strcmp(key, "bt_chain")) *value = h->bt_chain;
     else if (!strcmp(key, "hemm_waves")) *value = h->hemm_waves;
     else if (!strcmp(key, "bc_grid")) *value = h->bc_grid;
+    else if (!strcmp(key, "bc_variant")) *value = h->bc_variant;
     else if (!strcmp(key, "bc_dual_steps")) *value = h->bc_dual_steps;
     else if (!strcmp(key, "col_begin")) *value = h->col0;
     else if (!strcmp(key, "method")) *value = h->method;

@@ -28,6 +28,9 @@ constexpr int BC_LD = BC_B + 1;   // padded shared-memory leading dimension of t
 constexpr int BC_NT = 256;
 constexpr int BC_NW = BC_NT / 32;
 constexpr int BC_NC = BC_B / 4;   // columns per thread
+#ifndef BC_POLL_NS
+#define BC_POLL_NS 100
+#endif
 
 struct BcArgs {
     c128* band; int64_t ldab;
@@ -99,7 +102,7 @@ __device__ __forceinline__ void bc_st_release(int* p, int v) {
 }
 __device__ __forceinline__ void bc_poll(const int* progress, int sweep, int need) {
     if (sweep >= 0)
-        while (bc_ld_acquire(progress + sweep) < need) {}
+        while (bc_ld_acquire(progress + sweep) < need) { __nanosleep(BC_POLL_NS); }
 }
 // named barriers: 1 = compute group (BC_NT threads); 2, 3 = hand-off to the publisher warp (alternating)
 __device__ __forceinline__ void bc_sync_compute() { asm volatile("bar.sync 1, %0;" ::"n"(BC_NT) : "memory"); }
@@ -144,7 +147,7 @@ __device__ __forceinline__ c128 bc_make_reflector(c128 x, const BcStepCtx& t, in
 // PUB: a ninth (publisher) warp takes the release (one thread block per SM, 168 registers per thread); !PUB: thread 0 of the
 // compute group releases after a block barrier (two thread blocks of 8 warps per SM, 128 registers per thread: the second
 // block hides the latencies of the first -- used while the sweeps are long enough to keep 2 x 148 blocks busy).
-template <bool FULL, bool PUB>
+template <bool FULL, bool PUB, bool LEAN = !PUB>
 __device__ __forceinline__ bool bc_step(BcSmem& sm, const BcStepCtx& t, int r0, int len_, int len2_, int k, c128& tau, int& hb) {
     const int len = FULL ? BC_B : len_, len2 = FULL ? BC_B : len2_;
     const int r = t.r, q = t.q, rl = t.rl;
@@ -173,12 +176,12 @@ __device__ __forceinline__ bool bc_step(BcSmem& sm, const BcStepCtx& t, int r0, 
     bc_sync_compute();                                   // D landed; vs of this step visible
     // reflector entries of this thread's 16 columns: registers (PUB) or re-read from shared memory at every use (!PUB:
     // 64 registers fewer; a quarter warp reads one address, i.e. a broadcast)
-    c128 vcreg[PUB ? BC_NC : 1];
-    if constexpr (PUB) {
+    c128 vcreg[!LEAN ? BC_NC : 1];
+    if constexpr (!LEAN) {
 #pragma unroll
         for (int i = 0; i < BC_NC; ++i) vcreg[i] = sm.vs[q + 4 * i];
     }
-    auto vc = [&](int i) -> c128 { if constexpr (PUB) return vcreg[i]; else return sm.vs[q + 4 * i]; };
+    auto vc = [&](int i) -> c128 { if constexpr (!LEAN) return vcreg[i]; else return sm.vs[q + 4 * i]; };
     const c128 vr = sm.vs[r];
     // ---- the D phase (two-sided update of D_k) and the S phase (right update of S_{k+1}, next reflector) depend
     //      only on (v, tau): their matrix-vector products run in one loop, their block-wide reductions share one
@@ -337,7 +340,7 @@ __device__ __forceinline__ bool bc_step(BcSmem& sm, const BcStepCtx& t, int r0, 
         }
     }
     if (q == 0) {
-        t.Vj[(int64_t)(k + 1) * (32 * BC_B) + r] = vnr;          // zero beyond len2
+        __stcs(t.Vj + (int64_t)(k + 1) * (32 * BC_B) + r, vnr);  // zero beyond len2; write-once: streaming, keeps the band in L2
         sm.vs[r] = vnr;
     }
     if (t.tid == 0) t.tau2j[k + 1] = taun;
@@ -345,17 +348,27 @@ __device__ __forceinline__ bool bc_step(BcSmem& sm, const BcStepCtx& t, int r0, 
     return true;
 }
 
-template <bool PUB>
-__global__ void __launch_bounds__(PUB ? BC_NT + 32 : BC_NT, PUB ? 1 : 2) bulge_chase_kernel(const BcArgs a) {
+// VAR 0: publisher warp, one block per SM (default).  VAR 1: no publisher, lean registers, two blocks per SM (bc_dual_steps).
+// VAR 2: no publisher, one block per SM with the full register file (255 registers, no spills; option bc_variant = 2).
+// VAR 3: publisher warp AND the full register file for the compute warps: three warpgroups (8 compute warps, the publisher
+//        warp + 3 idle warps); the publisher's warpgroup gives its registers back (setmaxnreg.dec) and the compute
+//        warpgroups take them (setmaxnreg.inc 232), so the compute code needs no spills (option bc_variant = 3).
+template <int VAR>
+__global__ void __launch_bounds__(VAR == 3 ? BC_NT + 128 : VAR == 0 ? BC_NT + 32 : BC_NT, VAR == 1 ? 2 : 1) bulge_chase_kernel(const BcArgs a) {
+    constexpr bool PUB = VAR == 0 || VAR == 3, LEAN = VAR == 1;
     extern __shared__ __align__(16) unsigned char bc_raw[];
     BcSmem& sm = *reinterpret_cast<BcSmem*>(bc_raw);
 
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int N = a.N;
 
-    if (PUB && warp == BC_NW) {
+    if (PUB && warp >= BC_NW) {
         // ================= publisher warp: one release per step whose D phase is complete (the previous step is then
-        // complete in full), INT_MAX per completed sweep
+        // complete in full), INT_MAX per completed sweep.  (VAR 3: its whole warpgroup first hands its registers back.)
+        if constexpr (VAR == 3) {
+            asm volatile("setmaxnreg.dec.sync.aligned.u32 32;");
+            if (warp > BC_NW) return;
+        }
         int hb = 0;
         for (int j = a.j_begin + blockIdx.x; j < a.j_end; j += gridDim.x) {
             for (int k = 0;; ++k) {
@@ -368,6 +381,7 @@ __global__ void __launch_bounds__(PUB ? BC_NT + 32 : BC_NT, PUB ? 1 : 2) bulge_c
         }
         return;
     }
+    if constexpr (VAR == 3) asm volatile("setmaxnreg.inc.sync.aligned.u32 232;");
 
     BcStepCtx t;
     t.band = a.band; t.ldab = a.ldab;
@@ -395,7 +409,7 @@ __global__ void __launch_bounds__(PUB ? BC_NT + 32 : BC_NT, PUB ? 1 : 2) bulge_c
                 if (r < len) {
                     colj[1 + r] = (r == 0) ? cmake(beta, 0.0) : cmake(0.0, 0.0);
                 }
-                t.Vj[r] = vr;                                 // zero beyond len
+                __stcs(t.Vj + r, vr);                         // zero beyond len
                 sm.vs[r] = vr;
             }
             if (tid == 0) t.tau2j[0] = tau;
@@ -405,9 +419,10 @@ __global__ void __launch_bounds__(PUB ? BC_NT + 32 : BC_NT, PUB ? 1 : 2) bulge_c
             const int len = min(BC_B, N - r0);
             const int len2 = min(BC_B, N - (r0 + BC_B));
             // (the release of the step is handed to the publisher warp inside bc_step, after the D phase)
-            const bool more = (len == BC_B && len2 == BC_B) ? bc_step<true, PUB>(sm, t, r0, len, len2, k, tau, hb)
-                                                            : bc_step<false, PUB>(sm, t, r0, len, len2, k, tau, hb);
+            const bool more = (len == BC_B && len2 == BC_B) ? bc_step<true, PUB, LEAN>(sm, t, r0, len, len2, k, tau, hb)
+                                                            : bc_step<false, PUB, LEAN>(sm, t, r0, len, len2, k, tau, hb);
             if (!more) break;
+            // (one polling thread + a block barrier: eight polling warps measured 8 % slower -- they compete for the L2)
             if (tid == 0) bc_poll(a.progress, j - 1, k + 3);
             bc_sync_compute();
         }
@@ -430,6 +445,14 @@ __global__ void extract_tridiag_kernel(const c128* __restrict__ band, int64_t ld
     }
 }
 
+// zero the last stage (32 reflectors x 64 elements) of pass blockIdx.x
+__global__ void bc_zero_last_stage_kernel(c128* __restrict__ V2, const int64_t* __restrict__ pass_off) {
+    const int64_t first = pass_off[blockIdx.x], next = pass_off[blockIdx.x + 1];
+    if (next <= first) return;
+    c128* st = V2 + (next - 1) * (32 * BC_B);
+    for (int i = threadIdx.x; i < 32 * BC_B; i += blockDim.x) st[i] = cmake(0.0, 0.0);
+}
+
 int phase_band_to_tridiag(eigh_handle_s* h, c128* band, int64_t ldab, double* d, double* e, cudaStream_t s) {
     const int N = (int)h->N;
     if (h->b != BC_B) return set_err(h, -100, "bulge chasing is built for band width %d", BC_B);
@@ -437,11 +460,16 @@ int phase_band_to_tridiag(eigh_handle_s* h, c128* band, int64_t ldab, double* d,
     int* progress = ws_ptr<int>(h, pl.bc_progress);
     double* sgn = ws_ptr<double>(h, pl.sgn);
     EIGH_CUDA_OK(cudaMemsetAsync(progress, 0, (size_t)(N + 8) * sizeof(int), s));
-    // reflector slots that no (sweep, step) writes (short sweeps of a pass, sweeps beyond N-2) must read as zero
-    EIGH_CUDA_OK(cudaMemsetAsync(ws_ptr<c128>(h, pl.V2), 0, (size_t)v2_total_stages(N) * 32 * 64 * sizeof(c128), s));
     {
         const int rc = launch_pass_off(h, s);
         if (rc) return rc;
+    }
+    // Reflector slots that no (sweep, step) writes must read as zero.  Sweep j has ceil((N-1-j)/64) steps and a pass of 32
+    // sweeps has as many stages as its FIRST sweep has steps, so only the LAST stage of a pass can hold unwritten slots
+    // (later sweeps of the pass that are one step shorter, sweeps beyond N-2): 32 KB per pass instead of the whole array.
+    if (v2_npass(N) > 0) {
+        bc_zero_last_stage_kernel<<<(unsigned)v2_npass(N), 256, 0, s>>>(ws_ptr<c128>(h, pl.V2), ws_ptr<int64_t>(h, pl.pass_off));
+        ++h->launches;
     }
     if (N >= 2) {
         const size_t smem = sizeof(BcSmem);
@@ -461,7 +489,7 @@ int phase_band_to_tridiag(eigh_handle_s* h, c128* band, int64_t ldab, double* d,
         }
         void* kargs[] = {(void*)&a};
         if (j_switch > 0) {
-            auto kern = bulge_chase_kernel<false>;
+            auto kern = bulge_chase_kernel<1>;
             EIGH_CUDA_OK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
             int occ = 0;
             EIGH_CUDA_OK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kern, BC_NT, smem));
@@ -474,16 +502,18 @@ int phase_band_to_tridiag(eigh_handle_s* h, c128* band, int64_t ldab, double* d,
             ++h->launches;
         }
         if (j_switch < N - 1) {
-            auto kern = bulge_chase_kernel<true>;
+            const int var = h->bc_variant;
+            void (*kern)(const BcArgs) = var == 2 ? bulge_chase_kernel<2> : var == 3 ? bulge_chase_kernel<3> : bulge_chase_kernel<0>;
+            const int nthreads = var == 2 ? BC_NT : var == 3 ? BC_NT + 128 : BC_NT + 32;
             EIGH_CUDA_OK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
             int occ = 0;
-            EIGH_CUDA_OK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kern, BC_NT + 32, smem));
+            EIGH_CUDA_OK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kern, nthreads, smem));
             if (occ < 1) return set_err(h, EIGH_ERR_CUDA, "bulge_chase_kernel cannot be resident");
             int G = h->num_sms * occ;
             if (h->bc_grid > 0 && h->bc_grid < G) G = h->bc_grid;
             if (G > N - 1 - j_switch) G = N - 1 - j_switch;
             a.j_begin = j_switch; a.j_end = N - 1;
-            EIGH_CUDA_OK(cudaLaunchCooperativeKernel((void*)kern, dim3(G), dim3(BC_NT + 32), kargs, smem, s));
+            EIGH_CUDA_OK(cudaLaunchCooperativeKernel((void*)kern, dim3(G), dim3(nthreads), kargs, smem, s));
             ++h->launches;
         }
     }

@@ -49,6 +49,7 @@ struct eigh_handle_s {
     int hemm_waves;      // S1.3: split-K of HEMM-lower chosen for about this many thread blocks per SM
     int bt_chain;   // S4a: consecutive passes of one slab scheduled back to back (0 = auto)
     int bc_grid;    // S2: CTAs of the bulge-chasing kernel (0 = all that are co-resident)
+    int bc_variant;     // S2: 0 = publisher-warp kernel (default), 2 = no publisher warp, full register file
     int bc_dual_steps;  // S2: sweeps with at least this many chase steps run two thread blocks per SM (0 = never)
     int col0;       // first eigenvector column this handle returns (column shard of the back-transformations; default 0)
     int method;     // 2 = two-stage (default), 1 = one-stage direct tridiagonalisation

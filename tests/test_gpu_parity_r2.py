@@ -142,6 +142,9 @@ _OPTION_CASES = [
     ({"hemm_waves": 1}, 2100),
     ({"hemm_waves": 40}, 2100),
     ({"bc_grid": 7}, 2100),
+    ({"bc_variant": 0}, 2100),           # S2: publisher warp, 168 registers (the round-1 kernel)
+    ({"bc_variant": 2}, 2100),           # S2: no publisher warp, full register file
+    ({"bc_variant": 3}, 2100),           # S2: publisher warp + setmaxnreg (compute warps 224 registers)
     ({"bc_dual_steps": 1}, 2100),        # every sweep on the two-blocks-per-SM kernel
     ({"bc_dual_steps": 20}, 2100),       # long sweeps on the dual kernel, the rest on the publisher kernel
 ]
