@@ -8,7 +8,7 @@ back-transformations) over one synthetic matrix of BASELINE.json's `configs`.  D
 N = 49152 BdG vortex-tangle matrix (the largest single-GPU config and the north_star target).  BASELINE.json lists
 two runs for it, "full eigendecomposition and nev = N/2 subset": all eigenpairs are computed when W + K full solves
 fit the time budget (--time-budget, default 1500 s: the default W = 3, K = 2 run does), otherwise the nev = N/2 run is
-timed (the driver's --steps 20 --warmup 5: 25 x 75 s does not fit its 1800 s limit, 25 x 47 s does); which one ran is
+timed (the driver's --steps 20 --warmup 5: 25 x 72.5 s does not fit its 1800 s limit, 25 x 45.5 s does); which one ran is
 stated in `config.nev` / `config.nev_rule`.  The rule is a pure function of (config, W, K, budget), so both arms of
 the driver's comparison make the same choice.  The matrix is regenerated in place (eigh_assemble_bdg on the device, or
 a device copy of a pristine matrix for config 1) OUTSIDE the per-step CUDA-event brackets, because eigh_solve
@@ -44,7 +44,7 @@ CLOCK_QUERY = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.ac
 PHASES = ["p1_full_to_band", "p2_band_to_tridiag", "p3_tridiag_dc", "p4a_backtransform_band", "p4b_backtransform_full"]
 # seconds per eigh_solve (all eigenpairs) measured on one B200 for the nev rule; source: profiles/r01_summary.md and
 # profiles/r02_summary.md.  Only used to decide between the two runs BASELINE.json lists for configs 3 and 4.
-FULL_SOLVE_MODEL_S = {0: 0.03, 1: 0.2, 2: 0.6, 3: 14.0, 4: 75.0}
+FULL_SOLVE_MODEL_S = {0: 0.03, 1: 0.2, 2: 0.6, 3: 13.5, 4: 72.5}
 # executed real FP64 tensor flops per credited flop: GEMM engine in the 3M form = 6/8; bt_sweep_kernel: 116 DMMAs of
 # 512 flops per compact-WY block of 8 reflectors x 8 columns, credited 2 x 8 x 64 x 8 x 8
 EXECUTED_PER_CREDITED = {"p1": 0.75, "p4a": 116 * 512 / 65536.0, "p4b": 0.75}

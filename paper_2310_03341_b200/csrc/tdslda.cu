@@ -40,7 +40,7 @@ template <int MB, int MODE>
 __global__ void __launch_bounds__(TK_THREADS, MB <= 4 ? 2 : 1) kin_axis_kernel(const KinArgs p) {
     extern __shared__ __align__(16) unsigned char tk_raw[];
     constexpr int LP = 8 * MB, KS = 2 * MB, STAGES = tk_stages(MB);
-    constexpr bool A_IN_REGS = MB <= 4;
+    constexpr bool A_IN_REGS = MB <= 3;      // (MB = 4 with the fragments in registers spills at two blocks per SM)
     const int L = p.L;
     c128* buf = reinterpret_cast<c128*>(tk_raw);                  // [STAGES][u, v][LP][TK_PITCH]
     double* Ks = reinterpret_cast<double*>(buf + (size_t)2 * STAGES * LP * TK_PITCH);   // Ks[l * (LP + 1) + l2]
