@@ -242,3 +242,26 @@ def test_rgemm_syr2k_lower(geng, m, k):
     assert rel(out[low], ref[low]) < 1e-13
     skipped = torch.isnan(Cp)
     assert torch.isnan(out[skipped]).all()
+
+
+@pytest.mark.parametrize("real", [False, True])
+def test_one_stage_solve_host(real):
+    """eigh_solve_host on the 1-stage path, both element types (8-byte elements on the real path: the host <-> device
+    copies must use the working type's size): same answer as the device-resident solve, bit for bit."""
+    N = 300
+    H = rand_herm(N, 5100, real)
+    eng = _engine(N, real=real)
+    dt = torch.float64 if real else torch.complex128
+    Ah = torch.from_numpy(np.ascontiguousarray((H.real if real else H).T)).to(dt)
+    Wh = torch.empty(N, dtype=torch.float64)
+    Zh = torch.empty((N, N), dtype=dt)
+    At = torch.empty((N, N), dtype=dt, device="cuda")
+    W = torch.empty(N, dtype=torch.float64, device="cuda")
+    Zt = torch.empty((N, N), dtype=dt, device="cuda")
+    eng.solve_host(Ah, Wh, Zh, At, W, Zt)
+    W2, Zt2 = eng.solve(Ah.cuda())
+    torch.cuda.synchronize()
+    eng.close()
+    assert torch.equal(Wh, W2.cpu()) and torch.equal(Zh, Zt2.cpu())
+    _check(H.astype(np.complex128), Wh.numpy(), Zh.numpy().T.astype(np.complex128),
+           oracle.eigh(H.astype(np.complex128), vectors=False))
