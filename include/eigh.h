@@ -49,7 +49,8 @@ int eigh_create(eigh_handle_t* h, int64_t N, int64_t nev);
  * "hemm_waves" (S1.3: split-K of HEMM-lower sized for about this many thread blocks per SM; default 14),
  * "bt_chain" (S4a: consecutive passes of one column slab scheduled back to back so that followers read from L2;
  * 0 = automatic = 1, the unchained order), "bc_grid" (thread blocks of the S2 bulge-chasing kernel; 0 = every
- * co-resident block, the default), "bc_variant" (S2 kernel: 3 = publisher warp + register reallocation (setmaxnreg: the compute warps
+ * co-resident block, the default), "dgemm_mi" (real GEMM of the S3 merges: 8 = 64 x 32 warp tiles, 4 warps per
+ * thread block, the default; 4 = 32 x 32 warp tiles, 8 warps; process-wide like gemm_3m; identical results), "bc_variant" (S2 kernel: 3 = publisher warp + register reallocation (setmaxnreg: the compute warps
  * get 232 registers, no spills), the default; 2 = no publisher warp, full register file; 0 = publisher warp at 168 registers,
  * the round-1 kernel; all three give bit-identical results), "bc_dual_steps" (S2: sweeps with at least this many chase steps run on the variant
  * with two thread blocks per SM and no publisher warp; 0 = never, the default -- it measured 2-8 % slower at N = 27648 /

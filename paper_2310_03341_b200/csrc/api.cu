@@ -32,6 +32,7 @@ static size_t bump(size_t& off, size_t bytes) {
     return at;
 }
 
+extern int g_dgemm_mi;              // dgemm.cu
 size_t dc_arena_bytes(int64_t N);   // tridiag_dc.cu
 size_t dc_result_offset(int64_t N);
 size_t bt_scratch_bytes(const eigh_handle_s* h);   // bt_band.cu
@@ -155,6 +156,9 @@ int eigh_set_option(eigh_handle_t h, const char* key, int64_t value) {
     } else if (!strcmp(key, "bc_grid")) {
         if (value < 0 || value > 4096) return set_err(h, -3, "bc_grid must be in [0, 4096]");
         h->bc_grid = (int)value;
+    } else if (!strcmp(key, "dgemm_mi")) {
+        if (value != 4 && value != 8) return set_err(h, -3, "dgemm_mi must be 4 or 8");
+        g_dgemm_mi = (int)value;             // process-wide, like gemm_3m
     } else if (!strcmp(key, "bc_variant")) {
         if (value != 0 && value != 2 && value != 3) return set_err(h, -3, "bc_variant must be 0, 2 or 3");
         h->bc_variant = (int)value;

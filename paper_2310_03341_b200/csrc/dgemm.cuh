@@ -28,13 +28,16 @@ struct DgemmArgs {
     DgemmDesc one;
 };
 
-constexpr int DG_BM = 128, DG_BN = 64, DG_BK = 16, DG_STAGES = 4, DG_NT = 256;   // 108 KB of shared memory: 2 thread blocks per SM
+constexpr int DG_BM = 128, DG_BN = 64, DG_BK = 16, DG_STAGES = 4;   // 108 KB of shared memory: 2 thread blocks per SM
 constexpr int DG_SA = DG_BM + 4;     // As[k][m], stride == 4 (mod 16) doubles
 constexpr int DG_SB = DG_BK + 4;     // Bs[n][k]
 constexpr int DG_STAGE = DG_BK * DG_SA + DG_BN * DG_SB;    // doubles
 constexpr size_t DG_SMEM_BYTES = (size_t)DG_STAGES * DG_STAGE * sizeof(double);
 
-static __global__ void __launch_bounds__(DG_NT, 2) dgemm_kernel(const DgemmArgs p) {
+// MI = 8-row fragments per warp along M: 4 = warp tile 32 x 32, 8 warps (the default); 8 = warp tile 64 x 32, 4 warps
+template <int MI>
+static __global__ void __launch_bounds__(MI == 4 ? 256 : 128, 2) dgemm_kernel_t(const DgemmArgs p) {
+    constexpr int DG_NT = MI == 4 ? 256 : 128;
     extern __shared__ __align__(16) unsigned char dg_smem_raw[];
     double* smem = reinterpret_cast<double*>(dg_smem_raw);
 
@@ -56,11 +59,11 @@ static __global__ void __launch_bounds__(DG_NT, 2) dgemm_kernel(const DgemmArgs 
 
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int g = lane >> 2, t = lane & 3;
-    const int wm0 = (warp & 3) * 32, wn0 = (warp >> 2) * 32;   // 4 x 2 warps, warp tile 32 x 32
+    const int wm0 = MI == 4 ? (warp & 3) * 32 : (warp & 1) * 64, wn0 = (MI == 4 ? (warp >> 2) : (warp >> 1)) * 32;
 
-    double acc[4][4][2];
+    double acc[MI][4][2];
 #pragma unroll
-    for (int i = 0; i < 4; ++i)
+    for (int i = 0; i < MI; ++i)
 #pragma unroll
         for (int j = 0; j < 4; ++j) acc[i][j][0] = acc[i][j][1] = 0.0;
 
@@ -149,13 +152,13 @@ static __global__ void __launch_bounds__(DG_NT, 2) dgemm_kernel(const DgemmArgs 
         const double* Bs = As + DG_BK * DG_SA;
 #pragma unroll
         for (int kk = 0; kk < DG_BK; kk += 4) {
-            double a[4], b[4];
+            double a[MI], b[4];
 #pragma unroll
-            for (int i = 0; i < 4; ++i) a[i] = As[(kk + t) * DG_SA + wm0 + 8 * i + g];
+            for (int i = 0; i < MI; ++i) a[i] = As[(kk + t) * DG_SA + wm0 + 8 * i + g];
 #pragma unroll
             for (int j = 0; j < 4; ++j) b[j] = Bs[(wn0 + 8 * j + g) * DG_SB + kk + t];
 #pragma unroll
-            for (int i = 0; i < 4; ++i)
+            for (int i = 0; i < MI; ++i)
 #pragma unroll
                 for (int j = 0; j < 4; ++j) dmma884p(acc[i][j][0], acc[i][j][1], a[i], b[j]);
         }
@@ -163,7 +166,7 @@ static __global__ void __launch_bounds__(DG_NT, 2) dgemm_kernel(const DgemmArgs 
     cp_async_wait<0>();
 
 #pragma unroll
-    for (int i = 0; i < 4; ++i) {
+    for (int i = 0; i < MI; ++i) {
         const int row = m0 + wm0 + 8 * i + g;
 #pragma unroll
         for (int j = 0; j < 4; ++j)

@@ -142,6 +142,8 @@ _OPTION_CASES = [
     ({"hemm_waves": 1}, 2100),
     ({"hemm_waves": 40}, 2100),
     ({"bc_grid": 7}, 2100),
+    ({"dgemm_mi": 4}, 2100),             # S3 merges with the 32 x 32 warp tiles (round-1 kernel shape)
+    ({"dgemm_mi": 8}, 2100),             # ... and back to the default (the switch is process-wide)
     ({"bc_variant": 0}, 2100),           # S2: publisher warp, 168 registers (the round-1 kernel)
     ({"bc_variant": 2}, 2100),           # S2: no publisher warp, full register file
     ({"bc_variant": 3}, 2100),           # S2: publisher warp + setmaxnreg (compute warps 224 registers)
