@@ -354,3 +354,24 @@ def test_real_symmetric_input_gives_real_eigenvectors():
     p = wl.bdg_uniform((4, 4, 4), 0.5, 0.2)
     W4, Z4 = oracle.eigh(p.dense())
     assert np.abs(Z4.imag).max() == 0.0
+
+
+def test_ql_survives_the_underflow_split():
+    """The `r == 0` branch of the QL sweep (a rotation whose two components both underflow: split and restart) is only
+    reachable with subnormal data.  These two inputs reach it (found with an instrumented copy of the oracle; integers
+    times the smallest subnormal 5e-324, where every product rounds to an integer): no accuracy exists at that scale, so
+    the pin is what still must hold -- the routine terminates without failure, returns finite ascending values, and the
+    trace, which only involves exact additions there, is preserved.  A division by r = 0 would give NaN."""
+    den = 5e-324
+    for d, e in (([3, 0, -3, 2], [3, 3, 1]), ([0, -1, -1, -1, 0, 2], [3, 1, 3, 2, 2])):
+        dd, ee = np.array(d, dtype=np.float64) * den, np.array(e, dtype=np.float64) * den
+        W, Q = oracle.tridiag_ql(dd, ee)
+        assert np.isfinite(W).all() and np.isfinite(Q).all()
+        assert np.all(np.diff(W) >= 0)
+        assert W.sum() == dd.sum()
+        # the same matrix scaled into the normal range (exact scaling by 2^1000 / den) is solved to full accuracy
+        s = 2.0 ** 1000
+        Wn, Qn = oracle.tridiag_ql(np.array(d, dtype=np.float64) * s, np.array(e, dtype=np.float64) * s)
+        T = np.diag(np.array(d, float)) + np.diag(np.array(e, float), 1) + np.diag(np.array(e, float), -1)
+        assert np.abs(Wn / s - np.linalg.eigvalsh(T)).max() <= 1e-13 * np.abs(T).sum()
+        assert np.abs(Qn.T @ Qn - np.eye(len(d))).max() <= 1e-14
