@@ -79,6 +79,7 @@ template <typename T>
 struct HtSmem {
     T tile[HT_STG][HT_B * HT_LD];
     T vec[2][2][HT_B];        // [job parity][0: column-block vector v_J, 1: row-block vector v_I]
+    T vraw[HT_STG][2][HT_B];  // the entries of column c of A behind them, fetched with the tile (each by the thread that uses it)
     T red[2][4][HT_B];
     T xs[HT_B], ys[HT_B];
     T sred[HT_NT / 32];
@@ -243,20 +244,29 @@ __global__ void __launch_bounds__(HT_NT, 1) hetrd_panel_kernel(const HtArgs<T> a
             larfg_scalars<T>(alpha, xnorm2, tau, sc, beta);
         }
         if (cta == 0 && tid == 0) { a.e[c] = beta; a.tau[c] = tau; }
-        // v at global row gl (0 above the subdiagonal, 1 on it, scaled column below)
-        auto vget = [&](int gl) -> T {
+        // v at global row gl (0 above the subdiagonal, 1 on it, scaled column below), x = A(gl, c)
+        auto vmake = [&](int gl, T x) -> T {
             if (gl <= c || gl >= N) return S::zero();
             if (gl == c + 1) return S::one();
-            return S::mul(sc, ht_ldcg(a.A + gl + (int64_t)c * a.lda));
+            return S::mul(sc, x);
         };
         {
             // job list of this thread block: its tiles, then (V_I, W_I) of its row blocks
             const long long my_tiles = (ntiles > cta) ? (ntiles - cta + G - 1) / G : 0;
             const int my_blocks = (nblk > cta) ? (nblk - cta + G - 1) / G : 0;
             const long long njobs = my_tiles + (i > 0 ? 2LL * my_blocks : 0);
-            auto job_src = [&](long long j, int& I, int& J, int& kind, const T*& src, int64_t& ld, int& nr, int& nc) {
+            // tile cta + j G of this thread block, kept by increments (one decode per column, not one per job)
+            struct TileIt { int I, J; };
+            auto tile_next = [&](TileIt& t) {
+                t.I += G;
+                while (t.I >= nblk && t.J < nblk) { t.I -= nblk; ++t.J; t.I += t.J; }     // (past the last tile: stops at J = nblk)
+            };
+            TileIt it_issue, it_use;
+            ht_tile_decode(cta, nblk, it_issue.I, it_issue.J);
+            it_use = it_issue;
+            auto job_src = [&](long long j, const TileIt& t, int& I, int& J, int& kind, const T*& src, int64_t& ld, int& nr, int& nc) {
                 if (j < my_tiles) {
-                    ht_tile_decode(cta + j * G, nblk, I, J);
+                    I = t.I; J = t.J;
                     kind = (I == J) ? 1 : 0;
                     src = a.A + (j0 + I * HT_B) + (int64_t)(j0 + J * HT_B) * a.lda;
                     ld = a.lda;
@@ -277,8 +287,15 @@ __global__ void __launch_bounds__(HT_NT, 1) hetrd_panel_kernel(const HtArgs<T> a
                 if (j < njobs) {
                     int I, J, kind, nr, nc;
                     const T* src; int64_t ld;
-                    job_src(j, I, J, kind, src, ld, nr, nc);
+                    job_src(j, it_issue, I, J, kind, src, ld, nr, nc);
+                    if (j < my_tiles) tile_next(it_issue);
                     T* dst = sm.tile[j % HT_STG];
+                    if (kind == 0 && nr == HT_B && nc == HT_B) {          // interior tile: no predicates, addresses by increments
+                        const T* p = src + r + (int64_t)q * ld;
+                        T* dp = dst + q * HT_LD + r;
+#pragma unroll
+                        for (int it = 0; it < HT_B * HT_B / HT_NT; ++it) cp_async_elem(dp + it * 4 * HT_LD, p + (int64_t)(it * 4) * ld, true);
+                    } else
                     // diagonal tiles: only the lower triangle is read (the strict upper part is never valid input)
 #pragma unroll 4
                     for (int it = 0; it < HT_B * HT_B / HT_NT; ++it) {
@@ -288,6 +305,12 @@ __global__ void __launch_bounds__(HT_NT, 1) hetrd_panel_kernel(const HtArgs<T> a
                         const bool ok = rr < nr && cc < nc && (kind != 1 || rr >= cc) && (kind != 2 || I * HT_B + rr > cc);
                         cp_async_elem(dst + cc * HT_LD + rr, ok ? src + rr + (int64_t)cc * ld : src, ok);
                     }
+                    if (tid < 2 * HT_B) {                                 // this thread's entry of v_J (0) or v_I (1), in the same group
+                        const int which = tid >> 6;
+                        const int gl = j0 + (which ? I : J) * HT_B + r;
+                        const bool ok = gl > c + 1 && gl < N && !(kind >= 2 && which == 0);
+                        cp_async_elem(&sm.vraw[j % HT_STG][which][r], ok ? a.A + gl + (int64_t)c * a.lda : a.A, ok);
+                    }
                 }
                 cp_async_commit();
             };
@@ -295,14 +318,16 @@ __global__ void __launch_bounds__(HT_NT, 1) hetrd_panel_kernel(const HtArgs<T> a
             for (long long j = 0; j < njobs; ++j) {
                 int I, J, kind, nr, nc;
                 const T* src; int64_t ld;
-                job_src(j, I, J, kind, src, ld, nr, nc);
+                job_src(j, it_use, I, J, kind, src, ld, nr, nc);
+                if (j < my_tiles) tile_next(it_use);
                 const int par = (int)(j & 1);
-                if (tid < 2 * HT_B) {
+                cp_async_wait<HT_STG - 2>();
+                if (tid < 2 * HT_B) {                                 // (its own copy: visible to it after the wait)
                     const int which = tid >> 6;                       // 0: v_J, 1: v_I
                     const int blk = which ? I : J;
-                    sm.vec[par][which][r] = (kind >= 2 && which == 0) ? S::zero() : vget(j0 + blk * HT_B + r);
+                    sm.vec[par][which][r] = (kind >= 2 && which == 0) ? S::zero()
+                                                                      : vmake(j0 + blk * HT_B + r, sm.vraw[j % HT_STG][which][r]);
                 }
-                cp_async_wait<HT_STG - 2>();
                 __syncthreads();
                 issue(j + HT_STG - 1);
                 const T* St = sm.tile[j % HT_STG];
@@ -310,10 +335,17 @@ __global__ void __launch_bounds__(HT_NT, 1) hetrd_panel_kernel(const HtArgs<T> a
                 const T* vI = sm.vec[par][1];
                 T accr = S::zero(), accc = S::zero();
                 if (kind == 0) {
+                    // row r of A_IJ v_J and column r of A_IJ^H v_I, two accumulators each (independent FMA chains)
+                    T accr2 = S::zero(), accc2 = S::zero();
 #pragma unroll 4
-                    for (int cc = q; cc < HT_B; cc += 4) S::fma(accr, St[cc * HT_LD + r], vJ[cc]);          // row r of A_IJ v_J
-#pragma unroll 4
-                    for (int rr = q; rr < HT_B; rr += 4) S::fmac(accc, St[r * HT_LD + rr], vI[rr]);        // column r of A_IJ^H v_I
+                    for (int cc = q; cc < HT_B; cc += 8) {
+                        S::fma(accr, St[cc * HT_LD + r], vJ[cc]);
+                        S::fmac(accc, St[r * HT_LD + cc], vI[cc]);
+                        S::fma(accr2, St[(cc + 4) * HT_LD + r], vJ[cc + 4]);
+                        S::fmac(accc2, St[r * HT_LD + cc + 4], vI[cc + 4]);
+                    }
+                    accr = S::add(accr, accr2);
+                    accc = S::add(accc, accc2);
                 } else if (kind == 1) {
 #pragma unroll 4
                     for (int cc = q; cc < HT_B; cc += 4) {
@@ -400,7 +432,7 @@ __global__ void __launch_bounds__(HT_NT, 1) hetrd_panel_kernel(const HtArgs<T> a
                     if (act) {
                         const T y = S::add(S::add(sm.red[0][0][r], sm.red[0][1][r]), S::add(sm.red[0][2][r], sm.red[0][3][r]));
                         w = S::mul(tau, y);
-                        const T v = vget(gl);
+                        const T v = vmake(gl, (gl > c + 1 && gl < N) ? ht_ldcg(a.A + gl + (int64_t)c * a.lda) : S::zero());
                         S::fmac(dot, w, v);
                         a.A[gl + (int64_t)c * a.lda] = v;            // the reflector replaces the annihilated column
                     }
