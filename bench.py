@@ -239,6 +239,9 @@ def main():
                     help="order of the oracle's sample (about 10-30 s of CPU work on the box's host cores)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--host-buffers", default="pinned", choices=("pinned", "pageable"),
+                    help="e2e leg: host buffers page-locked in place (cudaHostRegister; falls back to pageable when the "
+                         "registration fails) or plain pageable memory through the handle's 2 x 256 MiB pinned ring")
     ap.add_argument("--no-epilogue", action="store_true")
     ap.add_argument("--context", action="store_true",
                     help="also time library routines on the same matrix as CONTEXT (never the target, never on the hot path): "
@@ -489,9 +492,11 @@ def main():
         except Exception as ex:   # reported, never hidden
             epilogue = dict(epilogue or {}, error=str(ex)[:200])
 
-    # ---- e2e: host buffers through eigh_solve_host.  A_host is PAGEABLE host memory of the full matrix; it is streamed
-    # H2D through the handle's bounded pinned ring (2 x 256 MiB), W and Z come back the same way; all of it inside the
-    # timed region (wall clock around the synchronous call, device idle on both sides).
+    # ---- e2e: host buffers through eigh_solve_host, H2D of the full matrix and D2H of W and Z inside the timed region
+    # (wall clock around the synchronous call, device idle on both sides).  Default: the host buffers are page-locked in
+    # place (cudaHostRegister, exact size, outside the timed region) and copied directly in 256 MiB chunks; with
+    # --host-buffers pageable (or when the registration fails) they stay pageable and are streamed through the handle's
+    # bounded pinned ring (2 x 256 MiB).
     e2e = None
     if not args.no_e2e and rank == 0:
         try:
@@ -501,6 +506,17 @@ def main():
             Ah.copy_(At)
             Wh = torch.empty(N, dtype=torch.float64)
             Zh = torch.empty((nev, N), dtype=wdt)
+            rt = torch.cuda.cudart()
+            registered = []
+            if args.host_buffers == "pinned":
+                for hb in (Ah, Zh, Wh):
+                    if int(rt.cudaHostRegister(hb.data_ptr(), hb.numel() * hb.element_size(), 0)) != 0:
+                        break
+                    registered.append(hb)
+                if len(registered) < 3:                 # all or nothing: report what the timed call really saw
+                    for hb in registered:
+                        rt.cudaHostUnregister(hb.data_ptr())
+                    registered = []
             times = []
             for i in range(2 if N <= 8192 else 1):
                 torch.cuda.synchronize()
@@ -510,8 +526,12 @@ def main():
                 times.append(time.perf_counter() - tt)
             e2e = {"value": min(times), "unit": "s", "h2d_bytes_per_step": mat_bytes,
                    "d2h_bytes_per_step": N * 8 + N * nev * (8 if args.real else 16),
-                   "host_buffers": "pageable, streamed through a 2 x 256 MiB pinned ring (eigh_solve_host)",
+                   "host_buffers": ("page-locked in place (cudaHostRegister), direct copies in 256 MiB chunks (eigh_solve_host)"
+                                    if registered else
+                                    "pageable, streamed through a 2 x 256 MiB pinned ring (eigh_solve_host)"),
                    "check_W_max_abs_diff": float((Wh - W.cpu()).abs().max().item())}
+            for hb in registered:
+                rt.cudaHostUnregister(hb.data_ptr())
             del Ah, Zh
         except Exception as ex:  # host allocation may fail for the largest configs
             e2e = {"value": None, "unit": "s", "error": str(ex)[:200]}
