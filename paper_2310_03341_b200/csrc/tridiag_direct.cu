@@ -60,6 +60,10 @@ static int gemm_t(eigh_handle_s* h, bool ta, bool tb, int M, int N, int K, doubl
 
 // ------------------------------------------------------------------ the panel kernel
 constexpr int HT_NT = 256, HT_B = 64, HT_LD = 65, HT_STG = 3;
+// The thread block = HT_NT compute threads + one LOADER warp (threads HT_NT .. HT_NTB-1) that only issues the asynchronous
+// copies of the tile phase: a copy instruction blocks its warp while the SM's queue of outstanding copies is full, and a
+// blocked compute warp holds up the block's barriers -- the loader warp takes that wait off the compute path.
+constexpr int HT_NTB = HT_NT + 32;
 
 template <typename T>
 struct HtArgs {
@@ -79,12 +83,38 @@ template <typename T>
 struct HtSmem {
     T tile[HT_STG][HT_B * HT_LD];
     T vec[2][2][HT_B];        // [job parity][0: column-block vector v_J, 1: row-block vector v_I]
-    T vraw[HT_STG][2][HT_B];  // the entries of column c of A behind them, fetched with the tile (each by the thread that uses it)
+    T vraw[HT_STG][2][HT_B];  // the entries of column c of A behind them, fetched with the tile
+    unsigned long long full[HT_STG], empty[HT_STG];   // mbarriers: the stage's copies have landed / its readers are done
     T red[2][4][HT_B];
     T xs[HT_B], ys[HT_B];
     T sred[HT_NT / 32];
     double dred[HT_NT / 32];
 };
+
+// barrier of the HT_NT compute threads (barrier 0 = the whole block incl. the loader warp: grid barriers only)
+__device__ __forceinline__ void ht_sync() { asm volatile("bar.sync 1, %0;" ::"n"(HT_NT) : "memory"); }
+__device__ __forceinline__ void ht_mbar_init(unsigned long long* b, int count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(b)), "r"(count));
+}
+__device__ __forceinline__ void ht_mbar_arrive(unsigned long long* b) {
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(b)) : "memory");
+}
+// arrives on b once every cp.async this thread has issued so far has landed (counts as one of the expected arrivals)
+__device__ __forceinline__ void ht_mbar_arrive_on_copies(unsigned long long* b) {
+    asm volatile("cp.async.mbarrier.arrive.noinc.shared::cta.b64 [%0];" ::"r"(smem_u32(b)) : "memory");
+}
+__device__ __forceinline__ void ht_mbar_wait(unsigned long long* b, unsigned parity) {
+    unsigned ok = 0;
+    while (!ok) {
+        asm volatile(
+            "{\n.reg .pred p;\n"
+            "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n"
+            "selp.u32 %0, 1, 0, p;\n}"
+            : "=r"(ok)
+            : "r"(smem_u32(b)), "r"(parity)
+            : "memory");
+    }
+}
 
 __device__ __forceinline__ void ht_grid_barrier(unsigned* ctr, unsigned target) {
     __syncthreads();
@@ -112,9 +142,9 @@ __device__ __forceinline__ double ht_block_sum_d(const double* src, int n, HtSme
     for (int i = threadIdx.x; i < n; i += HT_NT) s += __ldcg(src + i);
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
-    __syncthreads();
+    ht_sync();
     if ((threadIdx.x & 31) == 0) sm.dred[threadIdx.x >> 5] = s;
-    __syncthreads();
+    ht_sync();
     double t = 0.0;
 #pragma unroll
     for (int w = 0; w < HT_NT / 32; ++w) t += sm.dred[w];
@@ -131,9 +161,9 @@ __device__ __forceinline__ T ht_block_sum(const T* src, int n, HtSmem<T>& sm) {
     for (int i = threadIdx.x; i < n; i += HT_NT) s = S::add(s, ht_ldcg(src + i));
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) s = S::add(s, ht_shfl_xor(s, o));
-    __syncthreads();
+    ht_sync();
     if ((threadIdx.x & 31) == 0) sm.sred[threadIdx.x >> 5] = s;
-    __syncthreads();
+    ht_sync();
     T t = S::zero();
 #pragma unroll
     for (int w = 0; w < HT_NT / 32; ++w) t = S::add(t, sm.sred[w]);
@@ -155,7 +185,7 @@ __device__ __forceinline__ void ht_tile_decode(long long t, int nblk, int& I, in
 }
 
 template <typename T>
-__global__ void __launch_bounds__(HT_NT, 1) hetrd_panel_kernel(const HtArgs<T> a) {
+__global__ void __launch_bounds__(HT_NTB, 1) hetrd_panel_kernel(const HtArgs<T> a) {
     using S = Sc<T>;
     extern __shared__ __align__(16) unsigned char ht_raw[];
     HtSmem<T>& sm = *reinterpret_cast<HtSmem<T>*>(ht_raw);
@@ -169,9 +199,94 @@ __global__ void __launch_bounds__(HT_NT, 1) hetrd_panel_kernel(const HtArgs<T> a
     const bool tcta = cta == G - 1;
     unsigned epoch = 0;
 
+    if (tid == 0) {
+        for (int st = 0; st < HT_STG; ++st) { ht_mbar_init(&sm.full[st], 32); ht_mbar_init(&sm.empty[st], 1); }
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    __syncthreads();
+    // job list of this thread block in column i: its tiles (round robin over the column-strip order), then (V_I, W_I) of its
+    // row blocks.  The loader warp and the compute threads walk the same list.
+    const long long my_tiles = (ntiles > cta) ? (ntiles - cta + G - 1) / G : 0;
+    const int my_blocks = (nblk > cta) ? (nblk - cta + G - 1) / G : 0;
+    struct TileIt { int I, J; };
+    auto tile_next = [&](TileIt& t) {
+        t.I += G;
+        while (t.I >= nblk && t.J < nblk) { t.I -= nblk; ++t.J; t.I += t.J; }     // (past the last tile: stops at J = nblk)
+    };
+    auto job_src = [&](int i, long long j, const TileIt& t, int& I, int& J, int& kind, const T*& src, int64_t& ld, int& nr, int& nc) {
+        if (j < my_tiles) {
+            I = t.I; J = t.J;
+            kind = (I == J) ? 1 : 0;
+            src = a.A + (j0 + I * HT_B) + (int64_t)(j0 + J * HT_B) * a.lda;
+            ld = a.lda;
+            nr = min(HT_B, m - I * HT_B);
+            nc = min(HT_B, m - J * HT_B);
+        } else {
+            const long long jj = j - my_tiles;
+            I = cta + (int)(jj >> 1) * G;
+            J = 0;
+            kind = 2 + (int)(jj & 1);                      // 2: V_I, 3: W_I
+            nr = min(HT_B, m - I * HT_B);
+            nc = i;
+            if (kind == 2) { src = a.A + (j0 + I * HT_B) + (int64_t)j0 * a.lda; ld = a.lda; }
+            else { src = a.W + (j0 + I * HT_B); ld = a.ldw; }
+        }
+    };
+    unsigned jobno = 0;                          // jobs so far (all columns): stage jobno % HT_STG, use jobno / HT_STG of it
+
+    if (tid >= HT_NT) {
+        // ================= the loader warp: per column, between the same grid barriers as the tile phase
+        const int lane = tid - HT_NT;
+        for (int i = 0; i < a.nb; ++i) {
+            const int c = j0 + i;
+            ht_grid_barrier(a.counter, (++epoch) * (unsigned)G);
+            const long long njobs = my_tiles + (i > 0 ? 2LL * my_blocks : 0);
+            TileIt it;
+            ht_tile_decode(cta, nblk, it.I, it.J);
+            for (long long j = 0; j < njobs; ++j, ++jobno) {
+                int I, J, kind, nr, nc;
+                const T* src; int64_t ld;
+                job_src(i, j, it, I, J, kind, src, ld, nr, nc);
+                if (j < my_tiles) tile_next(it);
+                const int st = (int)(jobno % HT_STG);
+                if (jobno >= HT_STG) ht_mbar_wait(&sm.empty[st], ((jobno / HT_STG) - 1u) & 1u);     // its readers are done
+                T* dst = sm.tile[st];
+                if (kind == 0 && nr == HT_B && nc == HT_B) {              // interior tile: no predicates
+                    const T* p = src + lane;
+                    T* dp = dst + lane;
+#pragma unroll 8
+                    for (int cc = 0; cc < HT_B; ++cc) {
+                        cp_async_elem(dp + cc * HT_LD, p + (int64_t)cc * ld, true);
+                        cp_async_elem(dp + cc * HT_LD + 32, p + (int64_t)cc * ld + 32, true);
+                    }
+                } else {
+                    // diagonal tiles: only the lower triangle is read (the strict upper part is never valid input);
+                    // V_I: only the part strictly below the diagonal of A holds reflector entries
+#pragma unroll 4
+                    for (int e = 0; e < 2 * HT_B; ++e) {
+                        const int rr = lane + 32 * (e & 1), cc = e >> 1;
+                        const bool ok = rr < nr && cc < nc && (kind != 1 || rr >= cc) && (kind != 2 || I * HT_B + rr > cc);
+                        cp_async_elem(dst + cc * HT_LD + rr, ok ? src + rr + (int64_t)cc * ld : src, ok);
+                    }
+                }
+#pragma unroll
+                for (int e = 0; e < 4; ++e) {                               // entries of column c behind v_J (0) and v_I (1)
+                    const int which = e >> 1, rr = lane + 32 * (e & 1);
+                    const int gl = j0 + (which ? I : J) * HT_B + rr;
+                    const bool ok = gl > c + 1 && gl < N && !(kind >= 2 && which == 0);
+                    cp_async_elem(&sm.vraw[st][which][rr], ok ? a.A + gl + (int64_t)c * a.lda : a.A, ok);
+                }
+                ht_mbar_arrive_on_copies(&sm.full[st]);
+            }
+            ht_grid_barrier(a.counter, (++epoch) * (unsigned)G);
+            ht_grid_barrier(a.counter, (++epoch) * (unsigned)G);
+        }
+        return;
+    }
+
     if (tcta)      // the compact-WY factor is accumulated in place in global memory (read and written by this block only)
         for (int idx = tid; idx < HT_B * HT_B; idx += HT_NT) a.Tout[idx] = S::zero();
-    __syncthreads();
+    ht_sync();
 
     T tau_prev = S::zero();
     for (int i = 0; i <= a.nb; ++i) {
@@ -203,7 +318,7 @@ __global__ void __launch_bounds__(HT_NT, 1) hetrd_panel_kernel(const HtArgs<T> a
             sm.xs[tid] = S::conj(wck);
             sm.ys[tid] = S::conj(ht_ldcg(a.A + c + (int64_t)(j0 + tid) * a.lda));
         }
-        __syncthreads();                                         // (also orders the W fix before the reads below)
+        ht_sync();                                         // (also orders the W fix before the reads below)
         for (int I = cta; I < nblk; I += G) {
             const int gl = j0 + I * HT_B + r;
             const bool act = gl >= c && gl < N;
@@ -217,7 +332,7 @@ __global__ void __launch_bounds__(HT_NT, 1) hetrd_panel_kernel(const HtArgs<T> a
                 }
             }
             sm.red[0][q][r] = acc;
-            __syncthreads();
+            ht_sync();
             double pn = 0.0;
             if (q == 0 && act) {
                 const T sum = S::add(S::add(sm.red[0][0][r], sm.red[0][1][r]), S::add(sm.red[0][2][r], sm.red[0][3][r]));
@@ -230,7 +345,7 @@ __global__ void __launch_bounds__(HT_NT, 1) hetrd_panel_kernel(const HtArgs<T> a
 #pragma unroll
             for (int o = 16; o > 0; o >>= 1) pn += __shfl_xor_sync(0xffffffffu, pn, o);
             if ((tid & 31) == 0) sm.dred[tid >> 5] = pn;
-            __syncthreads();
+            ht_sync();
             if (tid == 0) a.nrm_part[I] = sm.dred[0] + sm.dred[1];
         }
         ht_grid_barrier(a.counter, (++epoch) * (unsigned)G);
@@ -251,86 +366,26 @@ __global__ void __launch_bounds__(HT_NT, 1) hetrd_panel_kernel(const HtArgs<T> a
             return S::mul(sc, x);
         };
         {
-            // job list of this thread block: its tiles, then (V_I, W_I) of its row blocks
-            const long long my_tiles = (ntiles > cta) ? (ntiles - cta + G - 1) / G : 0;
-            const int my_blocks = (nblk > cta) ? (nblk - cta + G - 1) / G : 0;
+            // the jobs of this column, in the order the loader warp issues them
             const long long njobs = my_tiles + (i > 0 ? 2LL * my_blocks : 0);
-            // tile cta + j G of this thread block, kept by increments (one decode per column, not one per job)
-            struct TileIt { int I, J; };
-            auto tile_next = [&](TileIt& t) {
-                t.I += G;
-                while (t.I >= nblk && t.J < nblk) { t.I -= nblk; ++t.J; t.I += t.J; }     // (past the last tile: stops at J = nblk)
-            };
-            TileIt it_issue, it_use;
-            ht_tile_decode(cta, nblk, it_issue.I, it_issue.J);
-            it_use = it_issue;
-            auto job_src = [&](long long j, const TileIt& t, int& I, int& J, int& kind, const T*& src, int64_t& ld, int& nr, int& nc) {
-                if (j < my_tiles) {
-                    I = t.I; J = t.J;
-                    kind = (I == J) ? 1 : 0;
-                    src = a.A + (j0 + I * HT_B) + (int64_t)(j0 + J * HT_B) * a.lda;
-                    ld = a.lda;
-                    nr = min(HT_B, m - I * HT_B);
-                    nc = min(HT_B, m - J * HT_B);
-                } else {
-                    const long long jj = j - my_tiles;
-                    I = cta + (int)(jj >> 1) * G;
-                    J = 0;
-                    kind = 2 + (int)(jj & 1);                      // 2: V_I, 3: W_I
-                    nr = min(HT_B, m - I * HT_B);
-                    nc = i;
-                    if (kind == 2) { src = a.A + (j0 + I * HT_B) + (int64_t)j0 * a.lda; ld = a.lda; }
-                    else { src = a.W + (j0 + I * HT_B); ld = a.ldw; }
-                }
-            };
-            auto issue = [&](long long j) {
-                if (j < njobs) {
-                    int I, J, kind, nr, nc;
-                    const T* src; int64_t ld;
-                    job_src(j, it_issue, I, J, kind, src, ld, nr, nc);
-                    if (j < my_tiles) tile_next(it_issue);
-                    T* dst = sm.tile[j % HT_STG];
-                    if (kind == 0 && nr == HT_B && nc == HT_B) {          // interior tile: no predicates, addresses by increments
-                        const T* p = src + r + (int64_t)q * ld;
-                        T* dp = dst + q * HT_LD + r;
-#pragma unroll
-                        for (int it = 0; it < HT_B * HT_B / HT_NT; ++it) cp_async_elem(dp + it * 4 * HT_LD, p + (int64_t)(it * 4) * ld, true);
-                    } else
-                    // diagonal tiles: only the lower triangle is read (the strict upper part is never valid input)
-#pragma unroll 4
-                    for (int it = 0; it < HT_B * HT_B / HT_NT; ++it) {
-                        const int idx = tid + it * HT_NT;
-                        const int rr = idx & 63, cc = idx >> 6;
-                        // (V_I: only the part strictly below the diagonal of A holds reflector entries)
-                        const bool ok = rr < nr && cc < nc && (kind != 1 || rr >= cc) && (kind != 2 || I * HT_B + rr > cc);
-                        cp_async_elem(dst + cc * HT_LD + rr, ok ? src + rr + (int64_t)cc * ld : src, ok);
-                    }
-                    if (tid < 2 * HT_B) {                                 // this thread's entry of v_J (0) or v_I (1), in the same group
-                        const int which = tid >> 6;
-                        const int gl = j0 + (which ? I : J) * HT_B + r;
-                        const bool ok = gl > c + 1 && gl < N && !(kind >= 2 && which == 0);
-                        cp_async_elem(&sm.vraw[j % HT_STG][which][r], ok ? a.A + gl + (int64_t)c * a.lda : a.A, ok);
-                    }
-                }
-                cp_async_commit();
-            };
-            for (int s = 0; s < HT_STG - 1; ++s) issue(s);
-            for (long long j = 0; j < njobs; ++j) {
+            TileIt it_use;
+            ht_tile_decode(cta, nblk, it_use.I, it_use.J);
+            for (long long j = 0; j < njobs; ++j, ++jobno) {
                 int I, J, kind, nr, nc;
                 const T* src; int64_t ld;
-                job_src(j, it_use, I, J, kind, src, ld, nr, nc);
+                job_src(i, j, it_use, I, J, kind, src, ld, nr, nc);
                 if (j < my_tiles) tile_next(it_use);
                 const int par = (int)(j & 1);
-                cp_async_wait<HT_STG - 2>();
-                if (tid < 2 * HT_B) {                                 // (its own copy: visible to it after the wait)
+                const int st = (int)(jobno % HT_STG);
+                ht_mbar_wait(&sm.full[st], (jobno / HT_STG) & 1u);     // the loader's copies of this stage have landed
+                if (tid < 2 * HT_B) {
                     const int which = tid >> 6;                       // 0: v_J, 1: v_I
                     const int blk = which ? I : J;
                     sm.vec[par][which][r] = (kind >= 2 && which == 0) ? S::zero()
-                                                                      : vmake(j0 + blk * HT_B + r, sm.vraw[j % HT_STG][which][r]);
+                                                                      : vmake(j0 + blk * HT_B + r, sm.vraw[st][which][r]);
                 }
-                __syncthreads();
-                issue(j + HT_STG - 1);
-                const T* St = sm.tile[j % HT_STG];
+                ht_sync();
+                const T* St = sm.tile[st];
                 const T* vJ = sm.vec[par][0];
                 const T* vI = sm.vec[par][1];
                 T accr = S::zero(), accc = S::zero();
@@ -361,7 +416,8 @@ __global__ void __launch_bounds__(HT_NT, 1) hetrd_panel_kernel(const HtArgs<T> a
                 }
                 sm.red[0][q][r] = accr;
                 sm.red[1][q][r] = accc;
-                __syncthreads();
+                ht_sync();
+                if (tid == 0) ht_mbar_arrive(&sm.empty[st]);          // every compute thread is past its reads of the stage
                 if (tid < 2 * HT_B) {
                     const int which = tid >> 6;
                     const T sum = S::add(S::add(sm.red[which][0][r], sm.red[which][1][r]),
@@ -375,7 +431,6 @@ __global__ void __launch_bounds__(HT_NT, 1) hetrd_panel_kernel(const HtArgs<T> a
                     }
                 }
             }
-            cp_async_wait<0>();
         }
         ht_grid_barrier(a.counter, (++epoch) * (unsigned)G);
 
@@ -389,14 +444,14 @@ __global__ void __launch_bounds__(HT_NT, 1) hetrd_panel_kernel(const HtArgs<T> a
                     for (int I = 0; I < nblk; ++I) s = S::add(s, ht_ldcg(a.g_part + ((size_t)I * 2 + which) * HT_B + r));
                 if (which == 0) sm.xs[r] = s; else sm.ys[r] = s;
             }
-            __syncthreads();
+            ht_sync();
             if (tcta) {
                 // T[0:i, i] = -tau T[0:i, 0:i] g2,  T[i, i] = tau
                 T acc = S::zero();
                 if (r < i)
                     for (int l = r + q; l < i; l += 4) S::fma(acc, a.Tout[r + (size_t)l * HT_B], sm.ys[l]);
                 sm.red[0][q][r] = acc;
-                __syncthreads();
+                ht_sync();
                 if (tid < HT_B) {
                     if (tid < i) {
                         const T sum = S::add(S::add(sm.red[0][0][tid], sm.red[0][1][tid]), S::add(sm.red[0][2][tid], sm.red[0][3][tid]));
@@ -405,7 +460,7 @@ __global__ void __launch_bounds__(HT_NT, 1) hetrd_panel_kernel(const HtArgs<T> a
                         a.Tout[tid + (size_t)i * HT_B] = tau;
                     }
                 }
-                __syncthreads();
+                ht_sync();
             }
             for (int I = cta; I < nblk; I += G) {
                 const int gl = j0 + I * HT_B + r;
@@ -425,7 +480,7 @@ __global__ void __launch_bounds__(HT_NT, 1) hetrd_panel_kernel(const HtArgs<T> a
                     }
                 }
                 sm.red[0][q][r] = S::sub(acc, corr);
-                __syncthreads();
+                ht_sync();
                 T dot = S::zero();
                 if (q == 0 && gl < N) {
                     T w = S::zero();
@@ -441,7 +496,7 @@ __global__ void __launch_bounds__(HT_NT, 1) hetrd_panel_kernel(const HtArgs<T> a
 #pragma unroll
                 for (int o = 16; o > 0; o >>= 1) dot = S::add(dot, ht_shfl_xor(dot, o));
                 if ((tid & 31) == 0) sm.sred[tid >> 5] = dot;
-                __syncthreads();
+                ht_sync();
                 if (tid == 0) a.dot_part[I] = S::add(sm.sred[0], sm.sred[1]);
             }
         }
@@ -484,7 +539,7 @@ static int tridiagonalise_direct_t(eigh_handle_s* h, T* A, int64_t lda, double* 
     auto kern = hetrd_panel_kernel<T>;
     EIGH_CUDA_OK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     int occ = 0;
-    EIGH_CUDA_OK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kern, HT_NT, smem));
+    EIGH_CUDA_OK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kern, HT_NTB, smem));
     if (occ < 1) return set_err(h, EIGH_ERR_CUDA, "hetrd_panel_kernel cannot be resident");
     if (N > 1) EIGH_CUDA_OK(cudaMemsetAsync(e, 0, (size_t)(N - 1) * sizeof(double), s));
     EIGH_CUDA_OK(cudaMemsetAsync(tau, 0, (size_t)N * sizeof(T), s));
@@ -503,7 +558,7 @@ static int tridiagonalise_direct_t(eigh_handle_s* h, T* A, int64_t lda, double* 
         a.W = W; a.ldw = N; a.e = e; a.tau = tau; a.Tout = T1 + (size_t)(j0 / HT_B) * HT_B * HT_B;
         a.counter = counter; a.nrm_part = nrm_part; a.dot_part = dot_part; a.g_part = g_part; a.Pl = Pl; a.Pu = Pu;
         void* kargs[] = {(void*)&a};
-        EIGH_CUDA_OK(cudaLaunchCooperativeKernel((void*)kern, dim3(G), dim3(HT_NT), kargs, smem, s));
+        EIGH_CUDA_OK(cudaLaunchCooperativeKernel((void*)kern, dim3(G), dim3(HT_NTB), kargs, smem, s));
         ++h->launches;
         const int mt = N - j0 - nb;                  // trailing order after the panel
         if (mt > 0) {
