@@ -60,10 +60,12 @@ static int gemm_t(eigh_handle_s* h, bool ta, bool tb, int M, int N, int K, doubl
 
 // ------------------------------------------------------------------ the panel kernel
 constexpr int HT_NT = 256, HT_B = 64, HT_LD = 65, HT_STG = 3;
-// The thread block = HT_NT compute threads + one LOADER warp (threads HT_NT .. HT_NTB-1) that only issues the asynchronous
-// copies of the tile phase: a copy instruction blocks its warp while the SM's queue of outstanding copies is full, and a
-// blocked compute warp holds up the block's barriers -- the loader warp takes that wait off the compute path.
-constexpr int HT_NTB = HT_NT + 32;
+// The thread block = HT_NT compute threads + HT_NL LOADER threads (threads HT_NT .. HT_NTB-1) that only issue the
+// asynchronous copies of the tile phase: a copy instruction blocks its warp while the SM's queue of outstanding copies is
+// full, and a blocked compute warp holds up the block's barriers -- the loader warps take that wait off the compute path.
+// (Four warps, not one: with one tile per thread block -- small matrices -- the time to issue a tile is exposed.)
+constexpr int HT_NL = 128;
+constexpr int HT_NTB = HT_NT + HT_NL;
 
 template <typename T>
 struct HtArgs {
@@ -200,7 +202,7 @@ __global__ void __launch_bounds__(HT_NTB, 1) hetrd_panel_kernel(const HtArgs<T> 
     unsigned epoch = 0;
 
     if (tid == 0) {
-        for (int st = 0; st < HT_STG; ++st) { ht_mbar_init(&sm.full[st], 32); ht_mbar_init(&sm.empty[st], 1); }
+        for (int st = 0; st < HT_STG; ++st) { ht_mbar_init(&sm.full[st], HT_NL); ht_mbar_init(&sm.empty[st], 1); }
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     __syncthreads();
@@ -235,8 +237,9 @@ __global__ void __launch_bounds__(HT_NTB, 1) hetrd_panel_kernel(const HtArgs<T> 
     unsigned jobno = 0;                          // jobs so far (all columns): stage jobno % HT_STG, use jobno / HT_STG of it
 
     if (tid >= HT_NT) {
-        // ================= the loader warp: per column, between the same grid barriers as the tile phase
-        const int lane = tid - HT_NT;
+        // ================= the loader warps: per column, between the same grid barriers as the tile phase
+        const int lt = tid - HT_NT;
+        const int lr = lt & 63, lq = lt >> 6;                  // row lr, columns lq, lq + 2, ...
         for (int i = 0; i < a.nb; ++i) {
             const int c = j0 + i;
             ht_grid_barrier(a.counter, (++epoch) * (unsigned)G);
@@ -252,29 +255,27 @@ __global__ void __launch_bounds__(HT_NTB, 1) hetrd_panel_kernel(const HtArgs<T> 
                 if (jobno >= HT_STG) ht_mbar_wait(&sm.empty[st], ((jobno / HT_STG) - 1u) & 1u);     // its readers are done
                 T* dst = sm.tile[st];
                 if (kind == 0 && nr == HT_B && nc == HT_B) {              // interior tile: no predicates
-                    const T* p = src + lane;
-                    T* dp = dst + lane;
+                    const T* p = src + lr + (int64_t)lq * ld;
+                    T* dp = dst + lq * HT_LD + lr;
 #pragma unroll 8
-                    for (int cc = 0; cc < HT_B; ++cc) {
-                        cp_async_elem(dp + cc * HT_LD, p + (int64_t)cc * ld, true);
-                        cp_async_elem(dp + cc * HT_LD + 32, p + (int64_t)cc * ld + 32, true);
-                    }
+                    for (int k = 0; k < HT_B * HT_B / HT_NL; ++k)
+                        cp_async_elem(dp + k * (HT_NL / HT_B) * HT_LD, p + (int64_t)(k * (HT_NL / HT_B)) * ld, true);
                 } else {
                     // diagonal tiles: only the lower triangle is read (the strict upper part is never valid input);
-                    // V_I: only the part strictly below the diagonal of A holds reflector entries
+                    // V_I: only the part strictly below the diagonal of A holds reflector entries.  Columns >= nc of a
+                    // (V_I, W_I) job are not written at all: their products are never used.
+                    const int ncl = kind >= 2 ? nc : HT_B;
 #pragma unroll 4
-                    for (int e = 0; e < 2 * HT_B; ++e) {
-                        const int rr = lane + 32 * (e & 1), cc = e >> 1;
-                        const bool ok = rr < nr && cc < nc && (kind != 1 || rr >= cc) && (kind != 2 || I * HT_B + rr > cc);
-                        cp_async_elem(dst + cc * HT_LD + rr, ok ? src + rr + (int64_t)cc * ld : src, ok);
+                    for (int cc = lq; cc < ncl; cc += HT_NL / HT_B) {
+                        const bool ok = lr < nr && cc < nc && (kind != 1 || lr >= cc) && (kind != 2 || I * HT_B + lr > cc);
+                        cp_async_elem(dst + cc * HT_LD + lr, ok ? src + lr + (int64_t)cc * ld : src, ok);
                     }
                 }
-#pragma unroll
-                for (int e = 0; e < 4; ++e) {                               // entries of column c behind v_J (0) and v_I (1)
-                    const int which = e >> 1, rr = lane + 32 * (e & 1);
-                    const int gl = j0 + (which ? I : J) * HT_B + rr;
+                {                                                           // entries of column c behind v_J (0) and v_I (1)
+                    const int which = lq;
+                    const int gl = j0 + (which ? I : J) * HT_B + lr;
                     const bool ok = gl > c + 1 && gl < N && !(kind >= 2 && which == 0);
-                    cp_async_elem(&sm.vraw[st][which][rr], ok ? a.A + gl + (int64_t)c * a.lda : a.A, ok);
+                    cp_async_elem(&sm.vraw[st][which][lr], ok ? a.A + gl + (int64_t)c * a.lda : a.A, ok);
                 }
                 ht_mbar_arrive_on_copies(&sm.full[st]);
             }
