@@ -85,6 +85,37 @@ def test_tridiagonalise_direct_against_the_oracle(N, real):
 
 
 @pytest.mark.parametrize("real", [False, True])
+@pytest.mark.parametrize("grid", [1, 2, 7, 40])
+def test_panel_kernel_grid_size_does_not_change_a_bit(grid, real):
+    """Option `ht_grid` (thread blocks of the cooperative panel kernel).  The per-tile partial products are stored per tile
+    and summed by the owner of a row block in a fixed order, so WHICH block computes a tile must not change any bit of d, e,
+    tau or the stored reflectors.  A small grid also makes every block walk the tile ring many times per column (N = 453:
+    36 tiles and up to 16 (V_I, W_I) jobs per column on 1-7 blocks): the loader warps' full / empty handshake wraps."""
+    N = 453
+    H = rand_herm(N, 2500, real)
+    outs = []
+    for g in (0, grid):                                      # 0 = the default (one block per SM, at most one per tile)
+        eng = _engine(N, real=real, **({"ht_grid": g} if g else {}))
+        At = _to_dev(H, real)
+        d = torch.full((N,), float("nan"), dtype=torch.float64, device="cuda")
+        e = torch.full((N,), float("nan"), dtype=torch.float64, device="cuda")
+        eng.tridiagonalise_direct(At, d, e)
+        torch.cuda.synchronize()
+        if g:
+            assert eng.get_option("ht_grid") == g
+        eng.close()
+        outs.append((d.clone(), e.clone(), At.clone()))
+    d0, e0, A0 = outs[0]
+    d1, e1, A1 = outs[1]
+    assert torch.equal(d0, d1) and torch.equal(e0[: N - 1], e1[: N - 1])
+    # stored reflectors: the lower triangle of A (column-major = the upper triangle of At); the rest is NaN input
+    iu = torch.triu_indices(N, N, device="cuda")
+    a0, a1 = A0[iu[0], iu[1]], A1[iu[0], iu[1]]
+    assert bool(torch.isfinite(torch.view_as_real(a0) if not real else a0).all())
+    assert torch.equal(torch.view_as_real(a0) if not real else a0, torch.view_as_real(a1) if not real else a1)
+
+
+@pytest.mark.parametrize("real", [False, True])
 @pytest.mark.parametrize("N", [1, 2, 3, 5, 31, 64, 65, 127, 130, 200, 333, 517, 1300])
 def test_one_stage_solve_small_and_ragged(N, real):
     H = rand_herm(N, 3000 + N, real)
