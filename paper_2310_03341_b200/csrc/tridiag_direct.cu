@@ -379,16 +379,22 @@ __global__ void __launch_bounds__(HT_NTB, 1) hetrd_panel_kernel(const HtArgs<T> 
                 const int par = (int)(j & 1);
                 const int st = (int)(jobno % HT_STG);
                 ht_mbar_wait(&sm.full[st], (jobno / HT_STG) & 1u);     // the loader's copies of this stage have landed
-                if (tid < 2 * HT_B) {
-                    const int which = tid >> 6;                       // 0: v_J, 1: v_I
-                    const int blk = which ? I : J;
-                    sm.vec[par][which][r] = (kind >= 2 && which == 0) ? S::zero()
-                                                                      : vmake(j0 + blk * HT_B + r, sm.vraw[st][which][r]);
+                // Every row of v_J and v_I below the subdiagonal entry (all but the tiles of the block row / column that
+                // holds column c): v = sc x there, so the products are taken with the fetched column entries x themselves
+                // and the sums scaled by sc -- no pass over the vectors, no barrier before the products.
+                const bool clean = j0 + (kind <= 1 ? J : I) * HT_B > c + 1;
+                if (!clean) {
+                    if (tid < 2 * HT_B) {
+                        const int which = tid >> 6;                       // 0: v_J, 1: v_I
+                        const int blk = which ? I : J;
+                        sm.vec[par][which][r] = (kind >= 2 && which == 0) ? S::zero()
+                                                                          : vmake(j0 + blk * HT_B + r, sm.vraw[st][which][r]);
+                    }
+                    ht_sync();
                 }
-                ht_sync();
                 const T* St = sm.tile[st];
-                const T* vJ = sm.vec[par][0];
-                const T* vI = sm.vec[par][1];
+                const T* vJ = clean ? sm.vraw[st][0] : sm.vec[par][0];
+                const T* vI = clean ? sm.vraw[st][1] : sm.vec[par][1];
                 T accr = S::zero(), accc = S::zero();
                 if (kind == 0) {
                     // row r of A_IJ v_J and column r of A_IJ^H v_I, two accumulators each (independent FMA chains)
@@ -421,8 +427,9 @@ __global__ void __launch_bounds__(HT_NTB, 1) hetrd_panel_kernel(const HtArgs<T> 
                 if (tid == 0) ht_mbar_arrive(&sm.empty[st]);          // every compute thread is past its reads of the stage
                 if (tid < 2 * HT_B) {
                     const int which = tid >> 6;
-                    const T sum = S::add(S::add(sm.red[which][0][r], sm.red[which][1][r]),
-                                         S::add(sm.red[which][2][r], sm.red[which][3][r]));
+                    T sum = S::add(S::add(sm.red[which][0][r], sm.red[which][1][r]),
+                                   S::add(sm.red[which][2][r], sm.red[which][3][r]));
+                    if (clean) sum = S::mul(sc, sum);
                     if (kind <= 1) {
                         const long long t = cta + j * G;
                         if (which == 0) a.Pl[t * HT_B + r] = sum;
