@@ -13,10 +13,11 @@
 //     The matrix-vector product A22 v reads the whole lower triangle once per column: 8/3 N^3 bytes (c128) in total, the
 //     HBM-bound half of the method -- roofline = bytes of lower-triangle tiles / time against HBM.
 //     ONE persistent cooperative kernel per panel: the 64 x 64 tiles of the lower triangle are dealt round-robin to the
-//     thread blocks and streamed through a 3-stage cp.async ring; a tile is used for both y_I += A_IJ v_J and
+//     thread blocks and streamed through a 3-stage cp.async ring filled by four LOADER warps (mbarrier full / empty
+//     handshake per stage; the 8 compute warps never issue a copy); a tile is used for both y_I += A_IJ v_J and
 //     y_J += A_IJ^H v_I; per-tile partial vectors are summed in a fixed order by the owner of each row block (no FP64
-//     atomics: bit-reproducible).  Three grid barriers per column (release/acquire counter).  The compact-WY factor T of
-//     the panel is accumulated on the fly from V^H v, which the step needs anyway.
+//     atomics: bit-reproducible, independent of the grid size).  Three grid barriers per column (release/acquire
+//     counter).  The compact-WY factor T of the panel is accumulated on the fly from V^H v, which the step needs anyway.
 // iii) Z <- Q Z with Q = H_0 H_1 ... H_{N-2}: panels merged 4 at a time into compact-WY blocks (K = 256) applied by
 //     the GEMM engine, as S4b does for the 2-stage path.
 #include <algorithm>
