@@ -85,7 +85,13 @@ int eigh_set_workspace(eigh_handle_t h, void* ws_dev, size_t bytes);
  *   W_dev : N doubles, all eigenvalues ascending.
  *   Z_dev : N x nev c128, ldz = N; column j = unit-2-norm eigenvector of W[j] (phase free).
  * Enqueues on `stream`; synchronises `stream` before returning (so that the failure count
- * can be returned). */
+ * can be returned).
+ * Scaling: eigh(s A) = s eigh(A) holds to rounding (exactly for s a power of two) as long as the
+ * SQUARES of the entries are representable, about 1e-150 <= max|a_ij| <= 1e150: the reductions form
+ * sums of squares without rescaling.  Beyond that range the call fails loudly (a positive return
+ * code: secular roots that did not converge); scale the matrix first.  S3 itself scales the
+ * tridiagonal matrix to norm ~1 by a power of two (its deflation test needs it) and is free of
+ * this limit (tested for s = 1e-200 .. 1e200). */
 int eigh_solve(eigh_handle_t h, void* A_dev, int64_t lda, double* W_dev, void* Z_dev,
                void* stream);
 
@@ -141,6 +147,8 @@ int eigh_band_to_tridiag(eigh_handle_t h, void* band_dev, int64_t ldab, double* 
  * d_dev[N], e_dev[N-1] are read (not modified); e may have either sign (the solver works on |e| and scales row i
  * of Q by prod_{t<i} sign(e_t), which maps the eigenvectors back to the signed matrix).  W_dev[N] ascending.
  * Q_dev: N x nev real FP64, ldq >= N, column j = eigenvector of W[j]; may alias no other argument.
+ * The matrix is scaled internally by the power of two next to max(|d|, |e|) (exact; the merge step's deflation
+ * test assumes a matrix of norm ~1, as in LAPACK's xSTEDC) and W scaled back.
  * Synchronises `stream`.  Returns the number of secular roots that failed to converge. */
 int eigh_tridiag_dc(eigh_handle_t h, const double* d_dev, const double* e_dev, double* W_dev,
                     double* Q_dev, int64_t ldq, void* stream);

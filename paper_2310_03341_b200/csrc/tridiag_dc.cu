@@ -33,7 +33,7 @@ constexpr int DC_LEAF_MAX = 32;
 // ------------------------------------------------------------------ arena
 struct DcBufs {
     double *QA, *QB, *U;              // ldq x N each
-    double *dcur, *dnew, *z, *dk, *zk, *mu, *lam, *zhat, *rot_c, *rot_s, *rho, *zsum, *esgn, *stats;
+    double *dcur, *dnew, *z, *dk, *zk, *mu, *lam, *zhat, *rot_c, *rot_s, *rho, *zsum, *esgn, *esc, *scale, *stats;
     int *perm, *nd_idx, *df_idx, *org, *rot_a, *rot_b, *kcount, *nrot, *fail, *bnd;
     int *ctype, *ktype, *upos, *acol, *k1c, *k2c;   // block structure of Q_old (column types, U row order)
     MergeDesc* desc;                  // all levels, concatenated
@@ -41,7 +41,7 @@ struct DcBufs {
     int64_t ldq;
 };
 
-static size_t dc_small_bytes(int64_t N) { return (size_t)(16 * 8 + 18 * 4) * (N + 64) + (size_t)(N + 64) * (sizeof(MergeDesc) + sizeof(DgemmDesc)) * 2 + 4096; }
+static size_t dc_small_bytes(int64_t N) { return (size_t)(16 * 8 + 18 * 4) * (N + 64) + (size_t)(N + 64) * (sizeof(MergeDesc) + sizeof(DgemmDesc)) * 2 + 16384; }   // (14 double + 15 int arrays, each rounded up to 256 bytes)
 
 size_t dc_arena_bytes(int64_t N) {
     const int64_t ldq = round_up(N, 8);
@@ -70,6 +70,8 @@ static DcBufs dc_carve(void* base, int64_t N) {
     b.lam = (double*)take(nd); b.zhat = (double*)take(nd); b.rot_c = (double*)take(nd);
     b.rot_s = (double*)take(nd); b.rho = (double*)take(nd); b.zsum = (double*)take(nd);
     b.esgn = (double*)take(nd);
+    b.esc = (double*)take(nd);
+    b.scale = (double*)take(256);
     b.stats = (double*)take(32 * 3 * sizeof(double));
     b.perm = (int*)take(ni); b.nd_idx = (int*)take(ni); b.df_idx = (int*)take(ni); b.org = (int*)take(ni);
     b.rot_a = (int*)take(ni); b.rot_b = (int*)take(ni); b.kcount = (int*)take(ni); b.nrot = (int*)take(ni);
@@ -82,10 +84,46 @@ static DcBufs dc_carve(void* base, int64_t N) {
 }
 
 // ------------------------------------------------------------------ S3.0 tearing
+// The deflation test of the merge step compares rho |z_i| with 8 eps max(|d|_max, |z|_max), z of unit norm: it assumes a
+// matrix of norm ~1 (LAPACK's xSTEDC scales to norm 1 before it calls the merge; without that a matrix of norm 1e-100
+// deflates everything and returns its diagonal).  scale[0] = the power of two next to max(|d|, |e|) -- the scaling is then
+// exact, and results for matrices of norm >= 1 are bit for bit what they were without it -- scale[1] = 1 / scale[0].
+__global__ void __launch_bounds__(1024) dc_norm_kernel(const double* __restrict__ d_in, const double* __restrict__ e_in, int N,
+                                                       double* __restrict__ scale) {
+    __shared__ double red[32];
+    double m = 0.0;
+    for (int i = threadIdx.x; i < N; i += 1024) {
+        m = fmax(m, fabs(d_in[i]));
+        if (i < N - 1) m = fmax(m, fabs(e_in[i]));
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) m = fmax(m, __shfl_xor_sync(0xffffffffu, m, o));
+    if ((threadIdx.x & 31) == 0) red[threadIdx.x >> 5] = m;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        for (int w = 1; w < 32; ++w) m = fmax(m, red[w]);
+        double sg = 1.0;
+        if (m > 0.0 && isfinite(m)) {
+            int ex;
+            frexp(m, &ex);                       // m = f 2^ex, f in [0.5, 1)
+            ex -= 1;                             // m / 2^ex in [1, 2)
+            if (ex > 1000) ex = 1000;            // (2^-ex must stay a normal number)
+            if (ex < -1000) ex = -1000;
+            sg = ldexp(1.0, ex);
+        }
+        scale[0] = sg;
+        scale[1] = 1.0 / sg;
+    }
+}
 __global__ void dc_tear_kernel(const double* __restrict__ d_in, const double* __restrict__ e_in, int N,
-                               const int* __restrict__ bnd, int L, double* __restrict__ dcur) {
+                               const int* __restrict__ bnd, int L, const double* __restrict__ scale, double* __restrict__ dcur,
+                               double* __restrict__ esc) {
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
-    if (i < N) dcur[i] = d_in[i];
+    const double inv = scale[1];
+    if (i < N) {
+        dcur[i] = d_in[i] * inv;
+        esc[i] = (i < N - 1) ? e_in[i] * inv : 0.0;
+    }
 }
 __global__ void dc_tear2_kernel(const double* __restrict__ e_in, const int* __restrict__ bnd, int L,
                                 double* __restrict__ dcur) {
@@ -616,10 +654,10 @@ __global__ void __launch_bounds__(256) dc_finish_kernel(const MergeDesc* __restr
 __global__ void __launch_bounds__(256) dc_output_kernel(int N, int col0, int nev, const int* __restrict__ perm, const double* __restrict__ dcur,
                                                         const double* __restrict__ Q, int64_t ldq, double* __restrict__ W,
                                                         double* __restrict__ Qout, int64_t ldo,
-                                                        const double* __restrict__ esgn) {
+                                                        const double* __restrict__ esgn, const double* __restrict__ scale) {
     const int rank = blockIdx.x;
     const int j = perm[rank];
-    if (threadIdx.x == 0) W[rank] = dcur[j];
+    if (threadIdx.x == 0) W[rank] = dcur[j] * scale[0];      // back from the unit-norm matrix (a power of two: exact)
     if (rank < col0 || rank >= col0 + nev) return;           // (col0 > 0: this handle's column shard)
     const double* a = Q + (int64_t)j * ldq;
     double* b = Qout + (int64_t)(rank - col0) * ldo;
@@ -672,11 +710,13 @@ int phase_tridiag_dc(eigh_handle_s* h, const double* d, const double* e, double*
     EIGH_CUDA_OK(cudaStreamSynchronize(st));   // host vectors go out of scope; copies are tiny
 
     // ---- tearing + leaves
-    dc_tear_kernel<<<(unsigned)ceil_div(N, 256), 256, 0, st>>>(d, e, N, B.bnd, L, B.dcur);
+    dc_norm_kernel<<<1, 1024, 0, st>>>(d, e, N, B.scale);
+    dc_tear_kernel<<<(unsigned)ceil_div(N, 256), 256, 0, st>>>(d, e, N, B.bnd, L, B.scale, B.dcur, B.esc);
+    e = B.esc;                                               // from here on: the scaled copy
     dc_tear2_kernel<<<(unsigned)ceil_div(L, 256), 256, 0, st>>>(e, B.bnd, L, B.dcur);
     dc_leaf_kernel<<<(unsigned)ceil_div(L, 4), 128, 0, st>>>(B.bnd, L, B.dcur, e, B.QA, ldq, B.fail);
     dc_esign_kernel<<<1, 1024, 0, st>>>(e, N, B.esgn);
-    h->launches += 4;
+    h->launches += 5;
 
     double* Qcur = B.QA;
     double* Qnew = B.QB;
@@ -724,7 +764,7 @@ int phase_tridiag_dc(eigh_handle_s* h, const double* d, const double* e, double*
     }
     // ---- final ascending order
     dc_rank_kernel<<<dim3((unsigned)ceil_div(N, 256), 1), 256, 0, st>>>(B.desc + final_desc, dcur, B.perm);
-    dc_output_kernel<<<N, 256, 0, st>>>(N, col0, nev, B.perm, dcur, Qcur, ldq, W, Qout, ldo, B.esgn);
+    dc_output_kernel<<<N, 256, 0, st>>>(N, col0, nev, B.perm, dcur, Qcur, ldq, W, Qout, ldo, B.esgn, B.scale);
     h->launches += 2;
     int fail = 0;
     double stats[32 * 3];

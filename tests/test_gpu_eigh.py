@@ -55,6 +55,24 @@ def test_small_and_ragged_sizes(N):
     check(H, W, Z, Wo)
 
 
+@pytest.mark.parametrize("method", [2, 1])
+@pytest.mark.parametrize("scale", [2.0 ** -333, 1e-140, 1e-100, 1e-3, 1e100, 1e140])
+def test_solve_of_a_scaled_matrix(method, scale):
+    """eigh(s H) = s eigh(H), same eigenvectors, for matrix norms far from 1 (the squares of the entries must stay
+    representable: include/eigh.h).  The merge step of the D&C deflates against 8 eps max(|d|_max, |z|_max) with a unit
+    vector z -- a test that assumes a matrix of norm ~1; S3 scales the tridiagonal matrix by a power of two first (as
+    LAPACK's xSTEDC does).  Without that a matrix of norm 1e-100 deflated everything: eigenvalue errors of 5 % of the
+    norm at full orthogonality, no error code.  Expected values: the oracle on the UNSCALED matrix."""
+    N = 200
+    H = rand_herm(N, 77)
+    Wo = oracle.eigh(H, vectors=False)
+    W, Z, _ = gpu_solve(H * scale, method=method)
+    check(H, W / scale, Z, Wo)
+    if scale == 2.0 ** -333:                      # a power of two: the whole solve scales exactly
+        W1, Z1, _ = gpu_solve(H, method=method)
+        assert np.array_equal(W / scale, W1) and np.array_equal(Z, Z1)
+
+
 def test_config0_closed_form_and_oracle():
     """Config 0: BdG uniform pairing 8x8x8 (N=1024), 64 distinct eigenvalues with multiplicity up to
     48: massive deflation.  Against the oracle and against the closed form."""

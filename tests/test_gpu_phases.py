@@ -185,6 +185,22 @@ def test_dc_random_and_subset(N, seed):
     assert np.linalg.norm(T @ Q2 - Q2 * W[None, :nev]) <= 1e-13 * np.linalg.norm(T)
 
 
+@pytest.mark.parametrize("scale", [2.0 ** -400, 1e-200, 1e-100, 1e-5, 1e5, 1e100, 1e200])
+def test_dc_scaled_tridiagonal(scale):
+    """eigh_tridiag_dc on s T: eigenvalues s W, the same eigenvectors.  The deflation test of the merge step assumes a
+    matrix of norm ~1 (tridiag_dc.cu scales by a power of two first, as xSTEDC does); without it a matrix of norm 1e-100
+    deflated completely and came back as its own diagonal.  A power-of-two s must reproduce the unscaled run bit for bit."""
+    rng = np.random.default_rng(11)
+    N = 500
+    d, e = rng.standard_normal(N), np.abs(rng.standard_normal(N - 1))
+    W1, Q1 = run_dc(d, e)
+    W, Q = run_dc(d * scale, e * scale)
+    check_tridiag(d, e, W / scale, Q)
+    assert np.abs(W / scale - W1).max() <= 1e-13 * np.abs(W1).max() * 5
+    if scale == 2.0 ** -400:
+        assert np.array_equal(W / scale, W1) and np.array_equal(Q, Q1)
+
+
 @pytest.mark.parametrize("nev_of", [lambda N: 1, lambda N: 7, lambda N: N // 2, lambda N: N - 1])
 def test_dc_subset_with_deflation_and_ties(nev_of):
     """nev < N shortens the last merge to the wanted secular roots: the subset must equal the leading columns of

@@ -375,3 +375,18 @@ def test_ql_survives_the_underflow_split():
         T = np.diag(np.array(d, float)) + np.diag(np.array(e, float), 1) + np.diag(np.array(e, float), -1)
         assert np.abs(Wn / s - np.linalg.eigvalsh(T)).max() <= 1e-13 * np.abs(T).sum()
         assert np.abs(Qn.T @ Qn - np.eye(len(d))).max() <= 1e-14
+
+
+@pytest.mark.parametrize("scale", [2.0 ** -333, 2.0 ** 333])
+def test_oracle_is_equivariant_under_power_of_two_scaling(scale):
+    """Every step of O1-O5 is homogeneous (reflectors, rotations, relative split tests): eigh(s H) = s eigh(H) BIT FOR BIT for a
+    power of two s while the squares of the entries stay representable.  A pin for any absolute threshold that might creep
+    in, and the expected values of the scaled-matrix GPU tests (tests/test_gpu_eigh.py::test_solve_of_a_scaled_matrix)."""
+    rng = np.random.default_rng(4242)
+    n = 60
+    A = rng.standard_normal((n, n)) + 1j * rng.standard_normal((n, n))
+    H = 0.5 * (A + A.conj().T)
+    W1, Z1 = oracle.eigh(H)
+    W2, Z2 = oracle.eigh(H * scale)
+    assert np.array_equal(W2 / scale, W1)
+    assert np.array_equal(Z2, Z1)
