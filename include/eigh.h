@@ -14,8 +14,9 @@
  *   - `stream` is a cudaStream_t passed as void* (0 = default stream).  Calls enqueue work
  *     on that stream only and may synchronise it (documented per call).
  *   - Return value: 0 success; -k = k-th argument invalid (nothing launched);
- *     +k = numerical failure count reported after completion (e.g. secular iterations that
- *     did not converge); EIGH_ERR_CUDA (= 1000 + cudaError_t) on a CUDA runtime error.
+ *     +k = numerical failure count reported after completion (secular iterations that did not
+ *     converge; capped at 999, eigh_last_error has the count -- non-finite input ends here, it
+ *     never hangs); EIGH_ERR_CUDA (= 1000 + cudaError_t) on a CUDA runtime error.
  *     eigh_last_error(h) gives a text description.
  *   - Ownership: the caller owns A, W, Z and the workspace (e.g. torch tensors); the handle
  *     owns only host-side plan data and a few CUDA events.  One handle per host thread.

@@ -303,7 +303,7 @@ int eigh_tridiag_dc(eigh_handle_t h, const double* d_dev, const double* e_dev, d
     rc = phase_tridiag_dc(h, d_dev, e_dev, W_dev, Q_dev, ldq, (cudaStream_t)stream, &nfail);
     if (rc) return cuda_fail(h, rc, "tridiag_dc");
     if (nfail) set_err(h, nfail, "%d secular roots did not converge", nfail);
-    return nfail;
+    return std::min(nfail, 999);          // (1000 and above are CUDA errors; the text has the count)
 }
 
 int eigh_backtransform_band(eigh_handle_t h, const double* Q_dev, int64_t ldq, void* Z_dev, int64_t ldz, void* stream) {
@@ -502,7 +502,7 @@ int eigh_solve(eigh_handle_t h, void* A_dev, int64_t lda, double* W_dev, void* Z
         h->phase_ms[1] = h->phase_ms[3] = 0.0;       // phases the 1-stage method does not have
         h->sweep_ms = 0.0;
         if (nfail) set_err(h, nfail, "%d secular roots did not converge", nfail);
-        return nfail;
+        return std::min(nfail, 999);
     }
     // NVTX ranges mark the host-side enqueue of every phase (the device-side spans are the CUDA events below)
     NvtxRange whole("eigh_solve");
@@ -541,7 +541,7 @@ int eigh_solve(eigh_handle_t h, void* A_dev, int64_t lda, double* W_dev, void* Z
         else (void)cudaGetLastError();
     }
     if (nfail) set_err(h, nfail, "%d secular roots did not converge", nfail);
-    return nfail;
+    return std::min(nfail, 999);          // (1000 and above are CUDA errors; the text has the count)
 }
 
 // ---- eigh_solve_host: host <-> device streaming through a bounded pinned ring -----------------------------------

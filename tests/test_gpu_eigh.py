@@ -140,6 +140,31 @@ def test_degenerate_inputs():
     assert np.abs(Z.conj().T @ Z - np.eye(N)).max() <= 1e-12 * N
 
 
+@pytest.mark.parametrize("method", [2, 1])
+@pytest.mark.parametrize("bad", [float("nan"), float("inf")])
+def test_non_finite_input_fails_loudly_and_returns(method, bad):
+    """A NaN or an infinity in the matrix: the call comes back (every iteration in the library is bounded) with a positive
+    return code below EIGH_ERR_CUDA = 1000 -- the failure count is capped at 999 so that it cannot be read as a CUDA error --
+    and a text that says what happened.  (Run under the suite's timeout: a hang here would be the bug.)"""
+    import ctypes
+    from paper_2310_03341_b200 import binding
+    N = 300
+    H = rand_herm(N, 99)
+    H[200, 17] = H[17, 200] = bad
+    eng = binding.Eigh(N, method=method)
+    At = torch.from_numpy(np.ascontiguousarray(H.T)).cuda()
+    W = torch.empty(N, dtype=torch.float64, device="cuda")
+    Zt = torch.empty((N, N), dtype=torch.complex128, device="cuda")
+    rc = eng.lib.eigh_solve(eng.h, ctypes.c_void_p(At.data_ptr()), N, ctypes.c_void_p(W.data_ptr()),
+                            ctypes.c_void_p(Zt.data_ptr()), None)
+    torch.cuda.synchronize()
+    assert 0 < rc < 1000, rc
+    assert "did not converge" in eng.last_error()
+    with pytest.raises(binding.EighError):
+        eng.solve(torch.from_numpy(np.ascontiguousarray(H.T)).cuda())
+    eng.close()
+
+
 @pytest.mark.parametrize("N", [130, 257, 389])
 @pytest.mark.parametrize("nev_of", [lambda N: 1, lambda N: 7, lambda N: 63, lambda N: 65, lambda N: N - 1])
 def test_ragged_subsets(N, nev_of):
